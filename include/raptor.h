@@ -1,0 +1,146 @@
+/* raptor.h -- C ABI of the B200-native RAPTOR hot path (arXiv:1801.10452, Bronzwaer et al. 2018).
+ *
+ * One image = for every pixel, backward RK4 integration of a Kerr null geodesic in modified
+ * Kerr-Schild coordinates fused with the covariant transfer update of I_nu/nu^3 along the ray.
+ * Citations are lines of the paper text with the equation they fall in; [A#] are the
+ * readings listed in DESIGN.md.  Plain pointers and sizes only; nothing throws across this
+ * boundary; no global state; a context is not thread-safe.
+ *
+ * Every function returns 0 (RAPTOR_OK) or a negative RAPTOR_E* code; raptor_last_error() gives
+ * the message.  "device" pointers are CUDA device memory of the current device, owned by the
+ * caller; "host" pointers are ordinary host memory.  Calls taking a cuda_stream (a cudaStream_t
+ * cast to void*, NULL = default stream) are asynchronous on that stream.
+ */
+#ifndef RAPTOR_B200_H
+#define RAPTOR_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RAPTOR_ABI_VERSION 1u
+
+enum {
+    RAPTOR_OK = 0,
+    RAPTOR_EINVAL = -1,        /* a parameter is out of range (message says which) */
+    RAPTOR_ENOMEM = -2,        /* device or host allocation failed */
+    RAPTOR_ECUDA = -3,         /* a CUDA call or kernel launch failed */
+    RAPTOR_EUNSUPPORTED = -4   /* valid request that this build does not implement */
+};
+
+/* plasma_model */
+enum { RAPTOR_VACUUM = 0, RAPTOR_SPHERE = 1, RAPTOR_TORUS = 2, RAPTOR_GRID2D = 3, RAPTOR_GRID3DT = 4, RAPTOR_SLAB = 5 };
+/* per-ray status word written by raptor_render */
+enum { RAPTOR_RUNNING = 0, RAPTOR_CAPTURED = 1, RAPTOR_ESCAPED = 2, RAPTOR_MAXSTEPS = 3, RAPTOR_THICK = 4, RAPTOR_NONFINITE = 5 };
+
+#define RAPTOR_MAX_FREQ 64
+
+typedef struct raptor_ctx raptor_ctx;   /* opaque; owns the device copies of the scene data */
+
+/* Statement of the problem (Table 2, Table B.1).
+ * POD, caller-owned, copied by raptor_create (including freq_hz[] and the grid). */
+typedef struct {
+    uint32_t struct_size;      /* = sizeof(raptor_params) */
+    uint32_t abi_version;      /* = RAPTOR_ABI_VERSION */
+    /* spacetime and chart: Kerr, M = 1, modified Kerr-Schild x = (t~, x1, x2, phi~), r = r0 + exp(x1),
+     * theta = pi x2 + (1-h)/2 sin(2 pi x2)  (A.10-A.11); h = 1: logarithmic KS */
+    double a;                  /* spin, |a| < 1 */
+    double mks_h;              /* 0 < h <= 1 */
+    double mks_r0;             /* r0 < r_H */
+    double mass;               /* mass parameter m multiplying every 2r of the metric: 1; 0 = flat space (tests) */
+    /* camera: Eq. 25-29, pixel centres alpha_ix = (ix+1/2) fov/nx - fov/2 [A4b] */
+    double r_cam;              /* camera radius [M], > r_H */
+    double incl_deg;           /* inclination, 0 < i < 180 (0 and 180 sit on the coordinate axis: rejected) */
+    double fov_M;              /* full width of the image plane [M] */
+    double t_cam;              /* coordinate time of the camera (slow light) */
+    /* physical scaling */
+    double M_bh_g;             /* black-hole mass [g]: L = G M / c^2 */
+    double D_src_cm;           /* distance [cm] */
+    double M_unit_g;           /* mass unit [g]: rho0 = M_unit / L^3 (grid models) */
+    /* integrator: RK4, Eq. 7-16, backward (d lambda = -h) [A2] */
+    double step_c, step_min, step_max;   /* policy A: h = clamp(c (r - r_H), min, max) (BASELINE.json configs[0]) */
+    double eps, delta;         /* policy B: Eq. 21-24 */
+    double eps_polar;          /* policy A polar guard: h <= eps_polar r |sin theta| (Eq. 23 with |k^theta| <= 1/r) */
+    double r_stop_in_factor;   /* stop when r < factor * r_H   (1.01) */
+    double r_stop_out_factor;  /* stop when r > factor * r_cam (1.1) */
+    double tau_cutoff;         /* stop when min_k tau_k exceeds it; +inf = off */
+    /* plasma */
+    double model[16];          /* SPHERE: n0, n_exp, T0[K], T_exp, beta.  TORUS: n_max, r_peak, r_halfwidth,
+                                  scale height H, T0, T_exp, beta.  SLAB: n_e, Theta_e, B[G], half thickness, sin(pitch) */
+    double tp_over_te;         /* T_p/T_e (Table 2) */
+    double gamma_ad;           /* adiabatic index of the grid fluid */
+    /* grid (GRID2D, GRID3DT): cell-centred, x1_i = x1_min + (i+1/2)(x1_max-x1_min)/n1, x2_j = (j+1/2)/n2,
+     * phi_k = (k+1/2) 2pi/n3, t_m = t0 + m dt_snap [A16] */
+    double x1_min, x1_max, t0, dt_snap;
+    const double *freq_hz;     /* host, n_freq observer frequencies [Hz] */
+    const void *grid_host;     /* host, AoS [nt][n1][n2][n3][8] = rho, u, u~1, u~2, u~3, B1, B2, B3 (HARM primitives) */
+    uint64_t grid_bytes;       /* must equal nt*n1*n2*n3*8*sizeof(element) */
+    int32_t nx, ny;            /* pixels */
+    int32_t integrator;        /* 0 = RK4 */
+    int32_t step_policy;       /* 0 = A, 1 = B */
+    int32_t max_steps;         /* per ray */
+    int32_t n_freq;            /* 1 .. RAPTOR_MAX_FREQ */
+    int32_t plasma_model;
+    int32_t k2_mode;           /* 0: K_2(1/Theta) = 2 Theta^2 */
+    int32_t n1, n2, n3, nt;
+    int32_t grid_dtype;        /* 0 = float64, 1 = float32 */
+    int32_t slow_light;        /* 1: interpolate between snapshots at the ray's coordinate time */
+    int32_t snapshot;          /* fast light: snapshot index used */
+    int32_t reserved_;
+} raptor_params;
+
+/* Validates and copies *p, uploads frequencies and grid.  *out is NULL on failure (then
+ * raptor_last_error(NULL) holds the thread-local message).  Synchronous. */
+int raptor_create(const raptor_params *p, raptor_ctx **out);
+
+/* Replaces the context's grid by a new one of identical shape (next snapshot series / movie frame).
+ * host -> device copy on the stream. */
+int raptor_upload_grid(raptor_ctx *ctx, const void *grid_host, uint64_t grid_bytes, void *cuda_stream);
+
+/* Steps a1-a7 of the hot path for the whole image:
+ *   d_image  device, [n_freq][ny][nx] float64: I_nu,obs in erg s^-1 cm^-2 Hz^-1 sr^-1 (Eq. 32)
+ *   d_status device, [ny][nx] int32 status word, or NULL
+ *   d_nsteps device, [ny][nx] int32 accepted RK4 steps of the ray, or NULL */
+int raptor_render(raptor_ctx *ctx, double *d_image, int32_t *d_status, int32_t *d_nsteps, void *cuda_stream);
+
+/* Render + flux reduction: d_flux_jy device [n_freq], F_k = 1e23 sum_pix I_k (fov/nx)(fov/ny) L^2/D^2 [Jy],
+ * summed in a fixed order (deterministic).  d_image_or_null: as d_image, or NULL to use scratch. */
+int raptor_spectrum(raptor_ctx *ctx, double *d_flux_jy, double *d_image_or_null, void *cuda_stream);
+
+/* Flux reduction alone of an image already on the device. */
+int raptor_flux(raptor_ctx *ctx, const double *d_image, double *d_flux_jy, void *cuda_stream);
+
+/* End-to-end convenience with HOST buffers: render on the context's own stream, copy image
+ * ([n_freq][ny][nx]), optional status / nsteps ([ny][nx]) and optional flux ([n_freq]) back, synchronise. */
+int raptor_render_host(raptor_ctx *ctx, double *h_image, int32_t *h_status, int32_t *h_nsteps, double *h_flux_jy);
+
+/* Diagnostics: trace n rays with given impact parameters (device arrays alpha[n], beta[n]) through the same
+ * device code as raptor_render.  Outputs (device, any may be NULL): I[n_freq][n], tau[n_freq][n], final
+ * state XK[n][8] = (X^0..3, K^0..3), status[n], nsteps[n]. */
+int raptor_trace(raptor_ctx *ctx, int32_t n, const double *d_alpha, const double *d_beta, double *d_I, double *d_tau,
+                 double *d_XK, int32_t *d_status, int32_t *d_nsteps, void *cuda_stream);
+
+/* Diagnostics: geodesic right-hand side f^a = -Gamma^a_bc k^b k^c (Eq. 6) at n points,
+ * d_XK[n][8] in, d_f[n][4] out (device). */
+int raptor_eval_rhs(raptor_ctx *ctx, int32_t n, const double *d_XK, double *d_f, void *cuda_stream);
+
+/* Counters accumulated by every render / trace since creation (synchronises the context's work):
+ * accepted RK4 steps, steps on which plasma was sampled, rays traced. */
+int raptor_get_counters(raptor_ctx *ctx, uint64_t *total_steps, uint64_t *sampled_steps, uint64_t *rays);
+
+/* Measures the FP64 FMA peak of the current device with independent DFMA chains on all SMs:
+ * *tflops = 2 * FMAs / time.  iters = chain length per thread (e.g. 1<<16). Synchronous. */
+int raptor_fp64_peak(int32_t iters, double *tflops, double *ms);
+
+int raptor_destroy(raptor_ctx *ctx);
+
+/* Message of the last failure on this context; ctx == NULL: of the last failed raptor_create /
+ * raptor_fp64_peak on this thread.  Never NULL. */
+const char *raptor_last_error(const raptor_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RAPTOR_B200_H */

@@ -1,0 +1,264 @@
+"""Thin ctypes binding of include/raptor.h -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of ``libraptor_b200.so``; PyTorch is used for
+device memory and streams.  There is no CPU fallback: if the library is missing, import of the
+library handle raises.  Function names mirror the C ABI (``raptor_create`` ... ``raptor_destroy``);
+``Raptor`` is a small RAII convenience around them.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libraptor_b200.so")
+ABI_VERSION = 1
+MAX_FREQ = 64
+
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
+STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 5: "NONFINITE"}
+
+# every symbol include/raptor.h declares
+SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_render", "raptor_spectrum", "raptor_flux",
+           "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_get_counters", "raptor_fp64_peak",
+           "raptor_destroy", "raptor_last_error")
+
+
+class RaptorParams(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("abi_version", C.c_uint32),
+        ("a", C.c_double), ("mks_h", C.c_double), ("mks_r0", C.c_double), ("mass", C.c_double),
+        ("r_cam", C.c_double), ("incl_deg", C.c_double), ("fov_M", C.c_double), ("t_cam", C.c_double),
+        ("M_bh_g", C.c_double), ("D_src_cm", C.c_double), ("M_unit_g", C.c_double),
+        ("step_c", C.c_double), ("step_min", C.c_double), ("step_max", C.c_double),
+        ("eps", C.c_double), ("delta", C.c_double), ("eps_polar", C.c_double),
+        ("r_stop_in_factor", C.c_double), ("r_stop_out_factor", C.c_double), ("tau_cutoff", C.c_double),
+        ("model", C.c_double * 16),
+        ("tp_over_te", C.c_double), ("gamma_ad", C.c_double),
+        ("x1_min", C.c_double), ("x1_max", C.c_double), ("t0", C.c_double), ("dt_snap", C.c_double),
+        ("freq_hz", C.POINTER(C.c_double)), ("grid_host", C.c_void_p), ("grid_bytes", C.c_uint64),
+        ("nx", C.c_int32), ("ny", C.c_int32), ("integrator", C.c_int32), ("step_policy", C.c_int32),
+        ("max_steps", C.c_int32), ("n_freq", C.c_int32), ("plasma_model", C.c_int32), ("k2_mode", C.c_int32),
+        ("n1", C.c_int32), ("n2", C.c_int32), ("n3", C.c_int32), ("nt", C.c_int32),
+        ("grid_dtype", C.c_int32), ("slow_light", C.c_int32), ("snapshot", C.c_int32), ("reserved_", C.c_int32),
+    ]
+
+
+class RaptorError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"raptor error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """The loaded shared library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1801_10452_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, u64p, dp = C.c_void_p, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_double)
+        L.raptor_create.argtypes = [C.POINTER(RaptorParams), C.POINTER(vp)]
+        L.raptor_upload_grid.argtypes = [vp, vp, C.c_uint64, vp]
+        L.raptor_render.argtypes = [vp, vp, vp, vp, vp]
+        L.raptor_spectrum.argtypes = [vp, vp, vp, vp]
+        L.raptor_flux.argtypes = [vp, vp, vp, vp]
+        L.raptor_render_host.argtypes = [vp, vp, vp, vp, vp]
+        L.raptor_trace.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.raptor_eval_rhs.argtypes = [vp, i32, vp, vp, vp]
+        L.raptor_get_counters.argtypes = [vp, u64p, u64p, u64p]
+        L.raptor_fp64_peak.argtypes = [i32, dp, dp]
+        L.raptor_destroy.argtypes = [vp]
+        L.raptor_last_error.argtypes = [vp]
+        L.raptor_last_error.restype = C.c_char_p
+        for name in SYMBOLS:
+            if name != "raptor_last_error":
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc, ctx=None):
+    if rc != 0:
+        raise RaptorError(rc, lib().raptor_last_error(ctx).decode())
+
+
+def params_from_scene(scene):
+    """Marshal a scene (duck-typed, see scenes.Scene) into a raptor_params; returns (params, keepalive)."""
+    p = RaptorParams()
+    p.struct_size = C.sizeof(RaptorParams)
+    p.abi_version = ABI_VERSION
+    for name in ("a", "mks_h", "mks_r0", "mass", "r_cam", "incl_deg", "fov_M", "t_cam", "M_bh_g", "D_src_cm",
+                 "M_unit_g", "step_c", "step_min", "step_max", "eps", "delta", "eps_polar", "r_stop_in_factor",
+                 "r_stop_out_factor", "tau_cutoff", "tp_over_te", "gamma_ad", "x1_min", "x1_max", "t0", "dt_snap"):
+        setattr(p, name, float(getattr(scene, name)))
+    for name in ("nx", "ny", "integrator", "step_policy", "max_steps", "plasma_model", "k2_mode",
+                 "n1", "n2", "n3", "nt", "grid_dtype", "slow_light", "snapshot"):
+        setattr(p, name, int(getattr(scene, name)))
+    m = list(scene.model) + [0.0] * 16
+    p.model = (C.c_double * 16)(*m[:16])
+    freq = np.ascontiguousarray(np.asarray(scene.freq_hz, dtype=np.float64))
+    p.n_freq = int(freq.size)
+    p.freq_hz = freq.ctypes.data_as(C.POINTER(C.c_double))
+    keep = [freq]
+    grid = getattr(scene, "grid", None)
+    if grid is not None:
+        g = np.ascontiguousarray(grid, dtype=np.float32 if scene.grid_dtype == 1 else np.float64)
+        p.grid_host = g.ctypes.data
+        p.grid_bytes = g.nbytes
+        keep.append(g)
+    return p, keep
+
+
+# ---- the C ABI, name for name ---------------------------------------------------------------
+def raptor_create(params: RaptorParams) -> C.c_void_p:
+    ctx = C.c_void_p()
+    _check(lib().raptor_create(C.byref(params), C.byref(ctx)))
+    return ctx
+
+
+def raptor_destroy(ctx):
+    _check(lib().raptor_destroy(ctx))
+
+
+def raptor_render(ctx, d_image, d_status=None, d_nsteps=None, stream=None):
+    _check(lib().raptor_render(ctx, d_image, d_status, d_nsteps, stream), ctx)
+
+
+def raptor_spectrum(ctx, d_flux, d_image=None, stream=None):
+    _check(lib().raptor_spectrum(ctx, d_flux, d_image, stream), ctx)
+
+
+def raptor_flux(ctx, d_image, d_flux, stream=None):
+    _check(lib().raptor_flux(ctx, d_image, d_flux, stream), ctx)
+
+
+def raptor_render_host(ctx, h_image, h_status=None, h_nsteps=None, h_flux=None):
+    _check(lib().raptor_render_host(ctx, h_image, h_status, h_nsteps, h_flux), ctx)
+
+
+def raptor_upload_grid(ctx, h_grid, nbytes, stream=None):
+    _check(lib().raptor_upload_grid(ctx, h_grid, nbytes, stream), ctx)
+
+
+def raptor_trace(ctx, n, d_alpha, d_beta, d_I=None, d_tau=None, d_XK=None, d_status=None, d_nsteps=None, stream=None):
+    _check(lib().raptor_trace(ctx, n, d_alpha, d_beta, d_I, d_tau, d_XK, d_status, d_nsteps, stream), ctx)
+
+
+def raptor_eval_rhs(ctx, n, d_XK, d_f, stream=None):
+    _check(lib().raptor_eval_rhs(ctx, n, d_XK, d_f, stream), ctx)
+
+
+def raptor_get_counters(ctx):
+    a, b, c = C.c_uint64(), C.c_uint64(), C.c_uint64()
+    _check(lib().raptor_get_counters(ctx, C.byref(a), C.byref(b), C.byref(c)), ctx)
+    return a.value, b.value, c.value
+
+
+def raptor_fp64_peak(iters: int = 1 << 16):
+    tf, ms = C.c_double(), C.c_double()
+    _check(lib().raptor_fp64_peak(int(iters), C.byref(tf), C.byref(ms)))
+    return tf.value, ms.value
+
+
+# ---- convenience wrapper ----------------------------------------------------------------------
+def _stream_ptr():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class Raptor:
+    """Context for one scene.  Outputs are torch CUDA tensors allocated here; the kernels fill them."""
+
+    def __init__(self, scene):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1801_10452_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.scene = scene
+        self.params, self._keep = params_from_scene(scene)
+        self.ctx = raptor_create(self.params)
+        self.nf, self.ny, self.nx = self.params.n_freq, self.params.ny, self.params.nx
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            raptor_destroy(self.ctx)
+            self.ctx = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def render(self, want_status=True, image=None):
+        import torch
+        dev = "cuda"
+        if image is None:
+            image = torch.empty((self.nf, self.ny, self.nx), dtype=torch.float64, device=dev)
+        status = torch.empty((self.ny, self.nx), dtype=torch.int32, device=dev) if want_status else None
+        nsteps = torch.empty((self.ny, self.nx), dtype=torch.int32, device=dev) if want_status else None
+        raptor_render(self.ctx, image.data_ptr(), status.data_ptr() if want_status else None,
+                      nsteps.data_ptr() if want_status else None, _stream_ptr())
+        return (image, status, nsteps) if want_status else image
+
+    def flux(self, image):
+        import torch
+        out = torch.empty((self.nf,), dtype=torch.float64, device="cuda")
+        raptor_flux(self.ctx, image.data_ptr(), out.data_ptr(), _stream_ptr())
+        return out
+
+    def spectrum(self, image=None):
+        import torch
+        out = torch.empty((self.nf,), dtype=torch.float64, device="cuda")
+        raptor_spectrum(self.ctx, out.data_ptr(), image.data_ptr() if image is not None else None, _stream_ptr())
+        return out
+
+    def render_host(self, want_status=False, want_flux=True):
+        image = np.empty((self.nf, self.ny, self.nx))
+        status = np.empty((self.ny, self.nx), dtype=np.int32) if want_status else None
+        nsteps = np.empty((self.ny, self.nx), dtype=np.int32) if want_status else None
+        flux = np.empty((self.nf,)) if want_flux else None
+        raptor_render_host(self.ctx, image.ctypes.data, status.ctypes.data if want_status else None,
+                           nsteps.ctypes.data if want_status else None, flux.ctypes.data if want_flux else None)
+        return dict(image=image, status=status, nsteps=nsteps, flux=flux)
+
+    def upload_grid(self, grid):
+        g = np.ascontiguousarray(grid, dtype=np.float32 if self.scene.grid_dtype == 1 else np.float64)
+        raptor_upload_grid(self.ctx, g.ctypes.data, g.nbytes, _stream_ptr())
+        import torch
+        torch.cuda.current_stream().synchronize()      # g may be a temporary
+
+    def trace(self, alpha, beta):
+        import torch
+        al = torch.as_tensor(np.asarray(alpha, dtype=np.float64)).cuda()
+        be = torch.as_tensor(np.asarray(beta, dtype=np.float64)).cuda()
+        n = al.numel()
+        I = torch.empty((self.nf, n), dtype=torch.float64, device="cuda")
+        tau = torch.empty((self.nf, n), dtype=torch.float64, device="cuda")
+        XK = torch.empty((n, 8), dtype=torch.float64, device="cuda")
+        status = torch.empty((n,), dtype=torch.int32, device="cuda")
+        nsteps = torch.empty((n,), dtype=torch.int32, device="cuda")
+        raptor_trace(self.ctx, n, al.data_ptr(), be.data_ptr(), I.data_ptr(), tau.data_ptr(), XK.data_ptr(),
+                     status.data_ptr(), nsteps.data_ptr(), _stream_ptr())
+        torch.cuda.synchronize()
+        return dict(I=I.cpu().numpy(), tau=tau.cpu().numpy(), XK=XK.cpu().numpy(),
+                    status=status.cpu().numpy(), nsteps=nsteps.cpu().numpy())
+
+    def eval_rhs(self, XK):
+        import torch
+        q = torch.as_tensor(np.ascontiguousarray(XK, dtype=np.float64)).cuda()
+        f = torch.empty((q.shape[0], 4), dtype=torch.float64, device="cuda")
+        raptor_eval_rhs(self.ctx, q.shape[0], q.data_ptr(), f.data_ptr(), _stream_ptr())
+        torch.cuda.synchronize()
+        return f.cpu().numpy()
+
+    def counters(self):
+        return raptor_get_counters(self.ctx)

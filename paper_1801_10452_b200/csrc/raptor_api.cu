@@ -1,0 +1,353 @@
+// raptor_api.cu -- the C ABI of include/raptor.h: validation, scene upload, launches.  Host code only.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/raptor.h"
+#include "raptor_kernels.h"
+
+using namespace raptor;
+
+struct raptor_ctx {
+    raptor_params p;
+    KP kp;
+    int device = 0, sm_count = 148;
+    void* d_grid = nullptr;
+    size_t grid_bytes = 0;
+    double* d_freq = nullptr;
+    unsigned int* d_queue = nullptr;
+    unsigned long long* d_counters = nullptr;
+    double* d_partial = nullptr;      // flux partial sums [n_freq][chunks]
+    double* d_scratch_image = nullptr;
+    double* d_scratch_flux = nullptr;
+    size_t scratch_pixels = 0;
+    cudaStream_t own_stream = nullptr;
+    char err[512] = {0};
+};
+
+static thread_local char g_err[512] = "";
+
+static int fail(raptor_ctx* ctx, int code, const char* fmt, ...) {
+    char* dst = ctx ? ctx->err : g_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+#define CK(ctx, call)                                                                                      \
+    do {                                                                                                   \
+        cudaError_t e_ = (call);                                                                           \
+        if (e_ != cudaSuccess)                                                                             \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? RAPTOR_ENOMEM : RAPTOR_ECUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                           \
+    } while (0)
+
+// theta(x2) of A.11 and its inverse by Newton-Raphson, A.14-A.16, on the lower half and mirrored
+// ([A22]: as printed the iteration cycles for theta near pi when h < 1).  Once per image, on the host.
+static double x2_of_theta(double h, double theta) {
+    const bool mirror = theta > 0.5 * kPI;
+    const double target = mirror ? kPI - theta : theta;
+    double x = 0.01;
+    for (int it = 0; it < 200; ++it) {
+        double f = kPI * x + 0.5 * (1.0 - h) * std::sin(2.0 * kPI * x) - target;      // A.15
+        double fp = kPI * (1.0 + (1.0 - h) * std::cos(2.0 * kPI * x));                // A.16
+        if (std::fabs(fp) < 1e-12) { x = 0.05; continue; }
+        double xn = x - f / fp;                                                       // A.14
+        if (xn < 0.0 || xn > 1.0) xn = 0.05;
+        bool done = std::fabs(xn - x) < 1e-15;
+        x = xn;
+        if (done) break;
+    }
+    return mirror ? 1.0 - x : x;
+}
+
+static size_t grid_elem_size(const raptor_params& p) { return p.grid_dtype == 1 ? sizeof(float) : sizeof(double); }
+static uint64_t grid_expected_bytes(const raptor_params& p) {
+    return (uint64_t)p.nt * p.n1 * p.n2 * p.n3 * 8ull * grid_elem_size(p);
+}
+
+static int validate(const raptor_params* p) {
+    if (!p) return fail(nullptr, RAPTOR_EINVAL, "params is NULL");
+    if (p->struct_size != sizeof(raptor_params)) return fail(nullptr, RAPTOR_EINVAL, "struct_size %u != %zu", p->struct_size, sizeof(raptor_params));
+    if (p->abi_version != RAPTOR_ABI_VERSION) return fail(nullptr, RAPTOR_EINVAL, "abi_version %u != %u", p->abi_version, RAPTOR_ABI_VERSION);
+    if (!(std::fabs(p->a) < 1.0)) return fail(nullptr, RAPTOR_EINVAL, "spin |a| must be < 1");
+    if (!(p->mass >= 0.0)) return fail(nullptr, RAPTOR_EINVAL, "mass parameter must be >= 0");
+    if (!(p->mks_h > 0.0 && p->mks_h <= 1.0)) return fail(nullptr, RAPTOR_EINVAL, "mks_h must be in (0,1]");
+    if (!(p->incl_deg > 0.0 && p->incl_deg < 180.0)) return fail(nullptr, RAPTOR_EINVAL, "inclination must be in (0,180) deg: 0 and 180 sit on the coordinate axis");
+    if (p->nx < 1 || p->ny < 1) return fail(nullptr, RAPTOR_EINVAL, "nx, ny must be >= 1");
+    if ((long long)p->nx * p->ny > (1ll << 31) - 64) return fail(nullptr, RAPTOR_EINVAL, "too many pixels");
+    if (p->n_freq < 1 || p->n_freq > RAPTOR_MAX_FREQ || !p->freq_hz) return fail(nullptr, RAPTOR_EINVAL, "n_freq must be 1..%d with freq_hz set", RAPTOR_MAX_FREQ);
+    for (int k = 0; k < p->n_freq; ++k)
+        if (!(p->freq_hz[k] > 0.0) || !std::isfinite(p->freq_hz[k])) return fail(nullptr, RAPTOR_EINVAL, "freq_hz[%d] must be positive", k);
+    double disc = p->mass * p->mass - p->a * p->a;
+    double rH = disc >= 0.0 ? p->mass + std::sqrt(disc) : 0.0;
+    if (!(p->r_cam > rH) || !(p->r_cam > p->mks_r0)) return fail(nullptr, RAPTOR_EINVAL, "r_cam must be outside the horizon");
+    if (!(p->mks_r0 < rH || p->mass == 0.0)) return fail(nullptr, RAPTOR_EINVAL, "mks_r0 must be < r_H");
+    if (!(p->fov_M > 0.0)) return fail(nullptr, RAPTOR_EINVAL, "fov_M must be > 0");
+    if (p->integrator != 0) return fail(nullptr, RAPTOR_EUNSUPPORTED, "integrator %d: only 0 (RK4) is built", p->integrator);
+    if (p->step_policy != 0 && p->step_policy != 1) return fail(nullptr, RAPTOR_EINVAL, "step_policy must be 0 or 1");
+    if (p->step_policy == 0 && !(p->step_min > 0.0 && p->step_max >= p->step_min && p->step_c >= 0.0 && p->eps_polar > 0.0))
+        return fail(nullptr, RAPTOR_EINVAL, "policy A needs 0 < step_min <= step_max, step_c >= 0, eps_polar > 0");
+    if (p->step_policy == 1 && !(p->eps > 0.0 && p->delta > 0.0)) return fail(nullptr, RAPTOR_EINVAL, "policy B needs eps > 0, delta > 0");
+    if (p->max_steps < 1) return fail(nullptr, RAPTOR_EINVAL, "max_steps must be >= 1");
+    if (!(p->r_stop_in_factor > 0.0) || !(p->r_stop_out_factor >= 1.0)) return fail(nullptr, RAPTOR_EINVAL, "bad r_stop factors");
+    if (std::isnan(p->tau_cutoff)) return fail(nullptr, RAPTOR_EINVAL, "tau_cutoff is NaN");
+    if (p->plasma_model < 0 || p->plasma_model > 5) return fail(nullptr, RAPTOR_EINVAL, "unknown plasma_model %d", p->plasma_model);
+    if (p->k2_mode != 0) return fail(nullptr, RAPTOR_EUNSUPPORTED, "k2_mode %d: only 0 (K2 = 2 Theta^2, PAPER.md:303) is built", p->k2_mode);
+    if (!(p->M_bh_g > 0.0) || !(p->D_src_cm > 0.0)) return fail(nullptr, RAPTOR_EINVAL, "M_bh_g and D_src_cm must be > 0");
+    if (p->plasma_model == RAPTOR_GRID2D || p->plasma_model == RAPTOR_GRID3DT) {
+        if (p->n1 < 2 || p->n2 < 2 || p->n3 < 1 || p->nt < 1) return fail(nullptr, RAPTOR_EINVAL, "grid dims: n1, n2 >= 2, n3, nt >= 1");
+        if (p->plasma_model == RAPTOR_GRID2D && (p->n3 != 1 || p->nt != 1 || p->grid_dtype != 0))
+            return fail(nullptr, RAPTOR_EINVAL, "GRID2D is [n1][n2][8] float64 (n3 = nt = 1)");
+        if (p->plasma_model == RAPTOR_GRID3DT && p->grid_dtype != 1)
+            return fail(nullptr, RAPTOR_EUNSUPPORTED, "GRID3DT is built for float32 cells (grid_dtype = 1)");
+        if (!(p->x1_max > p->x1_min)) return fail(nullptr, RAPTOR_EINVAL, "x1_max must be > x1_min");
+        if (!p->grid_host) return fail(nullptr, RAPTOR_EINVAL, "grid_host is NULL");
+        if (p->grid_bytes != grid_expected_bytes(*p)) return fail(nullptr, RAPTOR_EINVAL, "grid_bytes %llu != nt*n1*n2*n3*8*elem = %llu", (unsigned long long)p->grid_bytes, (unsigned long long)grid_expected_bytes(*p));
+        if (p->snapshot < 0 || p->snapshot >= p->nt) return fail(nullptr, RAPTOR_EINVAL, "snapshot out of range");
+        if (p->nt > 1 && p->slow_light && !(p->dt_snap > 0.0)) return fail(nullptr, RAPTOR_EINVAL, "dt_snap must be > 0");
+        if (!(p->M_unit_g > 0.0)) return fail(nullptr, RAPTOR_EINVAL, "M_unit_g must be > 0 for grid models");
+        if (!(p->gamma_ad > 1.0) || !(p->tp_over_te >= 0.0)) return fail(nullptr, RAPTOR_EINVAL, "gamma_ad > 1, tp_over_te >= 0");
+    }
+    return RAPTOR_OK;
+}
+
+static void build_kp(raptor_ctx* c) {
+    const raptor_params& p = c->p;
+    KP& k = c->kp;
+    std::memset(&k, 0, sizeof(k));
+    k.a = p.a; k.a2 = p.a * p.a; k.m = p.mass; k.omh = 1.0 - p.mks_h; k.r0 = p.mks_r0;
+    const double inc = p.incl_deg * (kPI / 180.0);
+    k.r_cam = p.r_cam; k.sin_i = std::sin(inc); k.cos_i = std::cos(inc);
+    k.sq1mc2 = std::sqrt(1.0 - k.cos_i * k.cos_i);
+    k.x1_cam = std::log(p.r_cam - p.mks_r0);
+    k.x2_cam = x2_of_theta(p.mks_h, inc);
+    k.dth_cam = kPI * (1.0 + (1.0 - p.mks_h) * std::cos(2.0 * kPI * k.x2_cam));
+    k.t_cam = p.t_cam;
+    k.fov = p.fov_M; k.pix_dx = p.fov_M / p.nx; k.pix_dy = p.fov_M / p.ny;
+    k.step_c = p.step_c; k.step_min = p.step_min; k.step_max = p.step_max;
+    k.eps = p.eps; k.delta = p.delta; k.eps_polar = p.eps_polar;
+    const double disc = p.mass * p.mass - p.a * p.a;
+    k.rH = disc >= 0.0 ? p.mass + std::sqrt(disc) : 0.0;
+    k.r_in = p.r_stop_in_factor * k.rH; k.r_out = p.r_stop_out_factor * p.r_cam;
+    k.tau_cutoff = p.tau_cutoff; k.use_tau_cutoff = std::isfinite(p.tau_cutoff) ? 1 : 0;
+    k.Lcm = kG * p.M_bh_g / (kC * kC);
+    const double rho0 = p.M_unit_g / (k.Lcm * k.Lcm * k.Lcm);
+    k.ne_scale = rho0 / (kMP + kME);                                     // Eq. 46
+    k.B0 = kC * std::sqrt(4.0 * kPI * rho0);
+    k.thetae_scale = (kMP / kME) * (p.gamma_ad - 1.0) / (1.0 + p.tp_over_te);
+    for (int i = 0; i < 16; ++i) k.model[i] = p.model[i];
+    if (p.n1 > 0) {
+        const double d1 = (p.x1_max - p.x1_min) / p.n1;
+        k.x1_first = p.x1_min + 0.5 * d1; k.inv_d1 = 1.0 / d1;
+    }
+    k.t0 = p.t0; k.inv_dt = p.dt_snap > 0.0 ? 1.0 / p.dt_snap : 0.0;
+    k.grid = c->d_grid; k.freq = c->d_freq;
+    k.nx = p.nx; k.ny = p.ny; k.step_policy = p.step_policy; k.max_steps = p.max_steps; k.n_freq = p.n_freq;
+    k.k2_mode = p.k2_mode; k.n1 = p.n1; k.n2 = p.n2; k.n3 = p.n3; k.nt = p.nt;
+    k.slow_light = p.slow_light; k.snapshot = p.snapshot;
+}
+
+extern "C" int raptor_create(const raptor_params* p, raptor_ctx** out) {
+    if (!out) return fail(nullptr, RAPTOR_EINVAL, "out is NULL");
+    *out = nullptr;
+    int rc = validate(p);
+    if (rc) return rc;
+    raptor_ctx* c = new (std::nothrow) raptor_ctx;
+    if (!c) return fail(nullptr, RAPTOR_ENOMEM, "host allocation failed");
+    c->p = *p;
+#define CKC(call)                                                                            \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess) {                                                             \
+            int code = fail(nullptr, e_ == cudaErrorMemoryAllocation ? RAPTOR_ENOMEM : RAPTOR_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+            raptor_destroy(c);                                                               \
+            return code;                                                                     \
+        }                                                                                    \
+    } while (0)
+    CKC(cudaGetDevice(&c->device));
+    CKC(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
+    CKC(cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking));
+    CKC(cudaMalloc(&c->d_freq, sizeof(double) * p->n_freq));
+    CKC(cudaMemcpy(c->d_freq, p->freq_hz, sizeof(double) * p->n_freq, cudaMemcpyHostToDevice));
+    CKC(cudaMalloc(&c->d_queue, sizeof(unsigned int)));
+    CKC(cudaMalloc(&c->d_counters, 3 * sizeof(unsigned long long)));
+    CKC(cudaMemset(c->d_counters, 0, 3 * sizeof(unsigned long long)));
+    const size_t npix = (size_t)p->nx * p->ny;
+    CKC(cudaMalloc(&c->d_partial, sizeof(double) * p->n_freq * (size_t)flux_chunks(npix)));
+    CKC(cudaMalloc(&c->d_scratch_flux, sizeof(double) * p->n_freq));
+    if (p->plasma_model == RAPTOR_GRID2D || p->plasma_model == RAPTOR_GRID3DT) {
+        c->grid_bytes = (size_t)p->grid_bytes;
+        CKC(cudaMalloc(&c->d_grid, c->grid_bytes));
+        CKC(cudaMemcpy(c->d_grid, p->grid_host, c->grid_bytes, cudaMemcpyHostToDevice));
+    }
+#undef CKC
+    c->p.freq_hz = nullptr;      // the context owns device copies only
+    c->p.grid_host = nullptr;
+    build_kp(c);
+    *out = c;
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_upload_grid(raptor_ctx* ctx, const void* grid_host, uint64_t grid_bytes, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (!ctx->d_grid) return fail(ctx, RAPTOR_EINVAL, "context has no grid");
+    if (!grid_host || grid_bytes != ctx->grid_bytes) return fail(ctx, RAPTOR_EINVAL, "grid_bytes %llu != %zu", (unsigned long long)grid_bytes, ctx->grid_bytes);
+    CK(ctx, cudaMemcpyAsync(ctx->d_grid, grid_host, ctx->grid_bytes, cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream));
+    return RAPTOR_OK;
+}
+
+static int run_rays(raptor_ctx* ctx, RenderOut& O, cudaStream_t s) {
+    O.queue = ctx->d_queue;
+    O.counters = ctx->d_counters;
+    CK(ctx, cudaMemsetAsync(ctx->d_queue, 0, sizeof(unsigned int), s));
+    CK(ctx, launch_render(ctx->kp, ctx->p.plasma_model, O, ctx->sm_count, s));
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_render(raptor_ctx* ctx, double* d_image, int32_t* d_status, int32_t* d_nsteps, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (!d_image) return fail(ctx, RAPTOR_EINVAL, "d_image is NULL");
+    RenderOut O;
+    std::memset(&O, 0, sizeof(O));
+    O.ntiles = (unsigned)(((ctx->p.nx + 7) / 8) * ((ctx->p.ny + 3) / 4));
+    O.image = d_image; O.status = d_status; O.nsteps = d_nsteps;
+    return run_rays(ctx, O, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int raptor_flux(raptor_ctx* ctx, const double* d_image, double* d_flux_jy, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (!d_image || !d_flux_jy) return fail(ctx, RAPTOR_EINVAL, "NULL buffer");
+    const raptor_params& p = ctx->p;
+    const double L = ctx->kp.Lcm;
+    const double scale = 1e23 * (p.fov_M / p.nx) * (p.fov_M / p.ny) * L * L / (p.D_src_cm * p.D_src_cm);
+    CK(ctx, launch_flux(d_image, (size_t)p.nx * p.ny, p.n_freq, scale, ctx->d_partial, d_flux_jy, (cudaStream_t)cuda_stream));
+    return RAPTOR_OK;
+}
+
+static int ensure_scratch(raptor_ctx* ctx) {
+    const size_t need = (size_t)ctx->p.nx * ctx->p.ny * ctx->p.n_freq;
+    if (ctx->scratch_pixels < need) {
+        if (ctx->d_scratch_image) cudaFree(ctx->d_scratch_image);
+        ctx->d_scratch_image = nullptr; ctx->scratch_pixels = 0;
+        CK(ctx, cudaMalloc(&ctx->d_scratch_image, need * sizeof(double)));
+        ctx->scratch_pixels = need;
+    }
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_spectrum(raptor_ctx* ctx, double* d_flux_jy, double* d_image_or_null, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (!d_flux_jy) return fail(ctx, RAPTOR_EINVAL, "d_flux_jy is NULL");
+    double* img = d_image_or_null;
+    if (!img) {
+        int rc = ensure_scratch(ctx);
+        if (rc) return rc;
+        img = ctx->d_scratch_image;
+    }
+    int rc = raptor_render(ctx, img, nullptr, nullptr, cuda_stream);
+    if (rc) return rc;
+    return raptor_flux(ctx, img, d_flux_jy, cuda_stream);
+}
+
+extern "C" int raptor_render_host(raptor_ctx* ctx, double* h_image, int32_t* h_status, int32_t* h_nsteps, double* h_flux_jy) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (!h_image) return fail(ctx, RAPTOR_EINVAL, "h_image is NULL");
+    int rc = ensure_scratch(ctx);
+    if (rc) return rc;
+    const size_t npix = (size_t)ctx->p.nx * ctx->p.ny;
+    cudaStream_t s = ctx->own_stream;
+    int32_t *d_status = nullptr, *d_nsteps = nullptr;
+    if (h_status) CK(ctx, cudaMallocAsync(&d_status, npix * sizeof(int32_t), s));
+    if (h_nsteps) CK(ctx, cudaMallocAsync(&d_nsteps, npix * sizeof(int32_t), s));
+    rc = raptor_render(ctx, ctx->d_scratch_image, d_status, d_nsteps, s);
+    if (!rc && h_flux_jy) rc = raptor_flux(ctx, ctx->d_scratch_image, ctx->d_scratch_flux, s);
+    if (!rc) {
+        CK(ctx, cudaMemcpyAsync(h_image, ctx->d_scratch_image, npix * ctx->p.n_freq * sizeof(double), cudaMemcpyDeviceToHost, s));
+        if (h_status) CK(ctx, cudaMemcpyAsync(h_status, d_status, npix * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+        if (h_nsteps) CK(ctx, cudaMemcpyAsync(h_nsteps, d_nsteps, npix * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+        if (h_flux_jy) CK(ctx, cudaMemcpyAsync(h_flux_jy, ctx->d_scratch_flux, ctx->p.n_freq * sizeof(double), cudaMemcpyDeviceToHost, s));
+    }
+    if (d_status) cudaFreeAsync(d_status, s);
+    if (d_nsteps) cudaFreeAsync(d_nsteps, s);
+    CK(ctx, cudaStreamSynchronize(s));
+    return rc;
+}
+
+extern "C" int raptor_trace(raptor_ctx* ctx, int32_t n, const double* d_alpha, const double* d_beta, double* d_I, double* d_tau,
+                            double* d_XK, int32_t* d_status, int32_t* d_nsteps, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (n < 0 || (n > 0 && (!d_alpha || !d_beta))) return fail(ctx, RAPTOR_EINVAL, "n < 0 or NULL alpha/beta");
+    if (n == 0) return RAPTOR_OK;
+    RenderOut O;
+    std::memset(&O, 0, sizeof(O));
+    O.ntiles = (unsigned)((n + 31) / 32);
+    O.alpha = d_alpha; O.beta = d_beta; O.nrays = n;
+    O.image = d_I; O.tau = d_tau; O.XK = d_XK; O.status = d_status; O.nsteps = d_nsteps;
+    return run_rays(ctx, O, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int raptor_eval_rhs(raptor_ctx* ctx, int32_t n, const double* d_XK, double* d_f, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (n < 0 || (n > 0 && (!d_XK || !d_f))) return fail(ctx, RAPTOR_EINVAL, "n < 0 or NULL buffer");
+    if (n == 0) return RAPTOR_OK;
+    CK(ctx, launch_eval_rhs(ctx->kp, n, d_XK, d_f, (cudaStream_t)cuda_stream));
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_get_counters(raptor_ctx* ctx, uint64_t* total_steps, uint64_t* sampled_steps, uint64_t* rays) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    unsigned long long h[3];
+    CK(ctx, cudaDeviceSynchronize());
+    CK(ctx, cudaMemcpy(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost));
+    if (total_steps) *total_steps = h[0];
+    if (sampled_steps) *sampled_steps = h[1];
+    if (rays) *rays = h[2];
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_fp64_peak(int32_t iters, double* tflops, double* ms) {
+    if (iters < 1 || !tflops) return fail(nullptr, RAPTOR_EINVAL, "iters < 1 or tflops NULL");
+    int dev = 0, sms = 0;
+    CK(nullptr, cudaGetDevice(&dev));
+    CK(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* d_out = nullptr;
+    CK(nullptr, cudaMalloc(&d_out, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CK(nullptr, cudaEventCreate(&e0));
+    CK(nullptr, cudaEventCreate(&e1));
+    const int blocks = sms * 8;
+    float best = 1e30f;
+    cudaError_t err = cudaSuccess;
+    for (int rep = 0; rep < 4 && err == cudaSuccess; ++rep) {       // rep 0 warms up
+        cudaEventRecord(e0, 0);
+        err = launch_fp64_peak(iters, blocks, d_out, 0);
+        cudaEventRecord(e1, 0);
+        if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+        float t = 0.f;
+        cudaEventElapsedTime(&t, e0, e1);
+        if (rep > 0 && t < best) best = t;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+    if (err != cudaSuccess) return fail(nullptr, RAPTOR_ECUDA, "fp64 probe: %s", cudaGetErrorString(err));
+    const double flops = 2.0 * 8.0 * (double)iters * 256.0 * (double)blocks;
+    *tflops = flops / (best * 1e-3) * 1e-12;
+    if (ms) *ms = best;
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_destroy(raptor_ctx* ctx) {
+    if (!ctx) return RAPTOR_OK;
+    cudaFree(ctx->d_grid); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_counters);
+    cudaFree(ctx->d_partial); cudaFree(ctx->d_scratch_image); cudaFree(ctx->d_scratch_flux);
+    if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    delete ctx;
+    return RAPTOR_OK;
+}
+
+extern "C" const char* raptor_last_error(const raptor_ctx* ctx) { return ctx ? ctx->err : g_err; }

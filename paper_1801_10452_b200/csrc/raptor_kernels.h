@@ -1,0 +1,32 @@
+// raptor_kernels.h -- host-visible launchers of raptor_kernels.cu (internal to the library).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "raptor_device.cuh"
+
+namespace raptor {
+
+// Outputs and work queue of one launch of the ray kernel.  All pointers are device pointers; any output may be NULL.
+struct RenderOut {
+    unsigned int* queue;            // tile counter, zeroed before the launch
+    unsigned int ntiles;
+    unsigned long long* counters;   // [3] steps, sampled steps, rays (accumulated)
+    const double* alpha;            // trace mode: explicit impact parameters [nrays]; NULL = render the pixel grid
+    const double* beta;
+    long long nrays;
+    double* image;                  // [n_freq][npix]
+    double* tau;                    // [n_freq][npix]
+    int32_t* status;                // [npix]
+    int32_t* nsteps;                // [npix]
+    double* XK;                     // [npix][8] final state
+};
+
+cudaError_t launch_render(const KP& P, int model, const RenderOut& O, int sm_count, cudaStream_t stream);
+int flux_chunks(size_t npix);
+cudaError_t launch_flux(const double* d_image, size_t npix, int n_freq, double scale, double* d_partial,
+                        double* d_flux, cudaStream_t stream);
+cudaError_t launch_eval_rhs(const KP& P, int n, const double* d_XK, double* d_f, cudaStream_t stream);
+cudaError_t launch_fp64_peak(int iters, int blocks, double* d_out, cudaStream_t stream);
+
+}  // namespace raptor
