@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- geodesic steps/s and images/s of the RAPTOR hot path on B200 (BASELINE.json metric).
+
+    python bench.py --gpus N --steps K --warmup W [--workload C2] [--impl reference]
+
+A "step" is one pass of the whole hot path (camera, geodesic RHS, RK4 + step rule,
+plasma sampler, fluid-frame quantities, emissivity/absorptivity/intensity update, image + flux reduction)
+over one synthetic image.  N = 1 workload: C2 = BASELINE.json configs[2], the 1024^2-pixel configuration
+the metric ("images/sec (1024^2 px)") is quoted on.  N > 1 (torchrun, one rank per GPU): rays are
+independent, so every rank renders its own frame (weak scaling, no data-path collective); value = all
+ranks' steps / max-over-ranks time.
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for the definitions of every key.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "geodesic_steps_per_sec"
+UNIT = "steps/s"
+
+# FP64 peak of one B200 for "bound": "alu": 148 SMs x 4 sub-partitions x 16 FP64 FMA
+# lanes x 2 flop x 1.965 GHz (clocks.max.sm).  The live DFMA probe (raptor_fp64_peak) is reported beside it.
+FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
+
+# FP64 flop per accepted RK4 step of each workload: thread-level executed DFMA x 2 +
+# DMUL + DADD of the shipped k_render kernel divided by the accepted steps, counted with ncu
+# (profiles/flop_per_step_r1.md).  It contains the 4 RHS evaluations with their exp / sin / cos, the RK4
+# combination and the sampled steps' share of sampler + transfer arithmetic.  Integer and control
+# instructions are not counted.  C3's figure is for its 32 frequencies.
+FLOP_PER_STEP = {"C0": 1610.9, "C1": 884.7, "C2": 1084.2, "C3": 1507.3, "C4": 1094.2}
+
+
+def build_scene(workload: str):
+    from paper_1801_10452_b200 import scenes
+    return scenes.config(workload)
+
+
+def algorithmic_flops(scene, workload, steps, sampled):
+    return steps * FLOP_PER_STEP[workload]
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(scene, row_stride, repeats=1):
+    """Times the oracle, as it stands, on every row_stride-th image row of the workload (host cores)."""
+    from oracle import oracle
+    o = oracle.Oracle(scene)
+    t0 = time.perf_counter()
+    steps = 0
+    for _ in range(repeats):
+        out = o.render(rows=(row_stride // 2, scene.ny), row_stride=row_stride)
+        steps += out["steps"]
+    dt = time.perf_counter() - t0
+    return steps, dt
+
+
+def omp_threads():
+    v = os.environ.get("OMP_NUM_THREADS")
+    return int(v) if v else (os.cpu_count() or 1)
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle (the only reference this tier has), bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scene = build_scene(args.workload)
+    stride = args.ref_row_stride or max(1, scene.ny // 8)     # 8 rows of the image per step
+    for _ in range(args.warmup):
+        oracle_sample(scene, max(stride, scene.ny // 2))
+    tot_steps, tot_t = 0, 0.0
+    for _ in range(args.steps):
+        s, dt = oracle_sample(scene, stride)
+        tot_steps += s
+        tot_t += dt
+    value = tot_steps / tot_t
+    sample = f"every {stride}th row of the {scene.nx}x{scene.ny} {args.workload} image per step ({scene.ny // stride} rows)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "pixels": [scene.nx, scene.ny], "n_freq": scene.n_freq,
+                       "note": "CPU oracle (oracle/raptor_oracle.c) as it stands, OpenMP over image rows"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": omp_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_1801_10452_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    binding.lib()
+
+    scene = build_scene(args.workload)
+    R = binding.Raptor(scene)
+    npix = scene.nx * scene.ny
+    image = torch.empty((scene.n_freq, scene.ny, scene.nx), dtype=torch.float64, device="cuda")
+    flux = torch.empty((scene.n_freq,), dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    sp = binding.C.c_void_p(stream.cuda_stream)
+    l2_flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_step(ev=None):
+        # a1-a6 + image write (render kernel), a7 flux reduction (2 small kernels): 3 launches
+        if ev:
+            ev[0].record(stream)
+        binding.raptor_render(R.ctx, image.data_ptr(), None, None, sp)
+        if ev:
+            ev[1].record(stream)
+        binding.raptor_flux(R.ctx, image.data_ptr(), flux.data_ptr(), sp)
+        if ev:
+            ev[2].record(stream)
+
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    torch.cuda.synchronize()
+    fp64_probe = binding.raptor_fp64_peak(1 << 16)[0] if rank == 0 else None
+    c_before = R.counters()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    events = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    barrier()
+    t_wall0 = time.perf_counter()
+    for k in range(args.steps):
+        l2_flush.zero_()                       # flush L2 between timed iterations (not timed)
+        one_step(events[k])
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop() if rank == 0 else None
+    step_ms = [e[0].elapsed_time(e[2]) for e in events]
+    render_ms = [e[0].elapsed_time(e[1]) for e in events]
+    c_after = R.counters()
+    steps_done = c_after[0] - c_before[0]
+    sampled_done = c_after[1] - c_before[1]
+    total_ms = sum(step_ms)
+
+    # ---- end to end through the C ABI with HOST buffers: grid upload (h2d), render, image + flux read back (d2h)
+    h_image = torch.empty((scene.n_freq, scene.ny, scene.nx), dtype=torch.float64).pin_memory()
+    h_flux = torch.empty((scene.n_freq,), dtype=torch.float64).pin_memory()
+    h_grid = None
+    if scene.grid is not None:
+        g = np.ascontiguousarray(scene.grid, dtype=np.float32 if scene.grid_dtype == 1 else np.float64)
+        h_grid = torch.from_numpy(g.reshape(-1).copy()).pin_memory()
+    e2e_steps = max(2, min(args.steps, 5))
+
+    def e2e_step():
+        if h_grid is not None:
+            binding.raptor_upload_grid(R.ctx, h_grid.data_ptr(), h_grid.numel() * h_grid.element_size(), None)
+        binding.raptor_render_host(R.ctx, h_image.data_ptr(), None, None, h_flux.data_ptr())
+
+    e2e_step()
+    barrier()
+    c0 = R.counters()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    c1 = R.counters()
+    e2e_units = c1[0] - c0[0]
+
+    # ---- aggregate over ranks: max time, summed units
+    agg = torch.tensor([total_ms, t_e2e * 1e3], dtype=torch.float64, device="cuda")
+    units = torch.tensor([float(steps_done), float(e2e_units)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(agg, op=dist.ReduceOp.MAX)
+        dist.all_reduce(units, op=dist.ReduceOp.SUM)
+    total_ms_max, e2e_ms_max = agg.tolist()
+    steps_all, e2e_units_all = units.tolist()
+
+    if rank == 0:
+        value = steps_all / (total_ms_max * 1e-3)
+        images_per_s = world * args.steps / (total_ms_max * 1e-3)
+        avg_render_ms = sum(render_ms) / len(render_ms)
+        flops_launch = algorithmic_flops(scene, args.workload, steps_done / args.steps, sampled_done / args.steps)
+        achieved = flops_launch / (avg_render_ms * 1e-3) / 1e12
+        # CPU baseline: the oracle on a bounded sample of the same workload (about 10-30 s of host work)
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            stride = max(1, scene.ny // 8)
+            s, dt = oracle_sample(scene, stride)
+            if dt < 5.0:
+                s2, dt2 = oracle_sample(scene, max(1, stride // 4))
+                s, dt, stride = s2, dt2, max(1, stride // 4)
+            cpu = {"value": s / dt, "unit": UNIT, "cores": omp_threads(), "kind": "oracle",
+                   "sample": f"every {stride}th row of the {scene.nx}x{scene.ny} {args.workload} image "
+                             f"({s} steps in {dt:.1f} s)"}
+        h2d = int(h_grid.numel() * h_grid.element_size()) if h_grid is not None else 0
+        d2h = int(h_image.numel() * 8 + h_flux.numel() * 8)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "pixels": [scene.nx, scene.ny], "n_freq": scene.n_freq,
+                       "spin": scene.a, "incl_deg": scene.incl_deg, "plasma_model": scene.plasma_model,
+                       "grid": [scene.nt, scene.n1, scene.n2, scene.n3], "l2": "flushed between timed iterations",
+                       "parallelism": f"frames x{world}" if world > 1 else "single GPU"},
+            "images_per_sec": images_per_s,
+            "steps_per_image": steps_done / args.steps, "sampled_steps_per_image": sampled_done / args.steps,
+            "clocks": clocks,
+            "e2e": {"value": e2e_units_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "images_per_sec": world * e2e_steps / (e2e_ms_max * 1e-3)},
+            "gpu_launches": 3 * args.steps,
+            "roofline": {"bound": "alu", "kernel": "k_render", "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
+                         "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None,
+                         "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md)",
+                         "fp64_probe_tflops": fp64_probe, "kernel_ms": avg_render_ms,
+                         "kernel_share_of_step": avg_render_ms / (total_ms / args.steps),
+                         "algorithmic_flop_per_launch": flops_launch},
+            "cpu_baseline": cpu,
+            "wall_s_timed_region": t_wall,
+        }
+        print(json.dumps(line))
+    R.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--ref-row-stride", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -105,6 +105,12 @@ int raptor_upload_grid(raptor_ctx *ctx, const void *grid_host, uint64_t grid_byt
  *   d_nsteps device, [ny][nx] int32 accepted RK4 steps of the ray, or NULL */
 int raptor_render(raptor_ctx *ctx, double *d_image, int32_t *d_status, int32_t *d_nsteps, void *cuda_stream);
 
+/* Multi-GPU sharding of one image: after this call raptor_render / raptor_spectrum /
+ * raptor_render_host trace only the 8x4-pixel tiles rank, rank + world, rank + 2 world, ... (row-major tile
+ * order) and leave every other pixel of the output buffers untouched.  Rays are independent, so the ranks'
+ * images (zero-initialised by the caller) sum to the full image exactly.  Default (0, 1) = whole image. */
+int raptor_set_shard(raptor_ctx *ctx, int32_t rank, int32_t world);
+
 /* Render + flux reduction: d_flux_jy device [n_freq], F_k = 1e23 sum_pix I_k (fov/nx)(fov/ny) L^2/D^2 [Jy],
  * summed in a fixed order (deterministic).  d_image_or_null: as d_image, or NULL to use scratch. */
 int raptor_spectrum(raptor_ctx *ctx, double *d_flux_jy, double *d_image_or_null, void *cuda_stream);

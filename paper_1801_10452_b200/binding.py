@@ -21,7 +21,7 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
 STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 5: "NONFINITE"}
 
 # every symbol include/raptor.h declares
-SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_render", "raptor_spectrum", "raptor_flux",
+SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_spectrum", "raptor_flux",
            "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_get_counters", "raptor_fp64_peak",
            "raptor_destroy", "raptor_last_error")
 
@@ -66,6 +66,7 @@ def lib():
         vp, i32, u64p, dp = C.c_void_p, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_double)
         L.raptor_create.argtypes = [C.POINTER(RaptorParams), C.POINTER(vp)]
         L.raptor_upload_grid.argtypes = [vp, vp, C.c_uint64, vp]
+        L.raptor_set_shard.argtypes = [vp, i32, i32]
         L.raptor_render.argtypes = [vp, vp, vp, vp, vp]
         L.raptor_spectrum.argtypes = [vp, vp, vp, vp]
         L.raptor_flux.argtypes = [vp, vp, vp, vp]
@@ -129,6 +130,10 @@ def raptor_destroy(ctx):
 
 def raptor_render(ctx, d_image, d_status=None, d_nsteps=None, stream=None):
     _check(lib().raptor_render(ctx, d_image, d_status, d_nsteps, stream), ctx)
+
+
+def raptor_set_shard(ctx, rank, world):
+    _check(lib().raptor_set_shard(ctx, int(rank), int(world)), ctx)
 
 
 def raptor_spectrum(ctx, d_flux, d_image=None, stream=None):
@@ -208,6 +213,9 @@ class Raptor:
         raptor_render(self.ctx, image.data_ptr(), status.data_ptr() if want_status else None,
                       nsteps.data_ptr() if want_status else None, _stream_ptr())
         return (image, status, nsteps) if want_status else image
+
+    def set_shard(self, rank, world):
+        raptor_set_shard(self.ctx, rank, world)
 
     def flux(self, image):
         import torch

@@ -16,6 +16,7 @@ struct raptor_ctx {
     raptor_params p;
     KP kp;
     int device = 0, sm_count = 148;
+    int shard_rank = 0, shard_world = 1;   // raptor_set_shard
     void* d_grid = nullptr;
     size_t grid_bytes = 0;
     double* d_freq = nullptr;
@@ -205,6 +206,7 @@ extern "C" int raptor_upload_grid(raptor_ctx* ctx, const void* grid_host, uint64
 static int run_rays(raptor_ctx* ctx, RenderOut& O, cudaStream_t s) {
     O.queue = ctx->d_queue;
     O.counters = ctx->d_counters;
+    if (O.tile_stride == 0) { O.tile_offset = 0; O.tile_stride = 1; }
     CK(ctx, cudaMemsetAsync(ctx->d_queue, 0, sizeof(unsigned int), s));
     CK(ctx, launch_render(ctx->kp, ctx->p.plasma_model, O, ctx->sm_count, s));
     return RAPTOR_OK;
@@ -215,9 +217,20 @@ extern "C" int raptor_render(raptor_ctx* ctx, double* d_image, int32_t* d_status
     if (!d_image) return fail(ctx, RAPTOR_EINVAL, "d_image is NULL");
     RenderOut O;
     std::memset(&O, 0, sizeof(O));
-    O.ntiles = (unsigned)(((ctx->p.nx + 7) / 8) * ((ctx->p.ny + 3) / 4));
+    const unsigned all_tiles = (unsigned)(((ctx->p.nx + 7) / 8) * ((ctx->p.ny + 3) / 4));
+    // shard: rank r of w takes tiles r, r+w, r+2w, ... (interleaved so that shadow and torus spread evenly)
+    O.tile_offset = (unsigned)ctx->shard_rank; O.tile_stride = (unsigned)ctx->shard_world;
+    O.ntiles = all_tiles > O.tile_offset ? (all_tiles - O.tile_offset + O.tile_stride - 1) / O.tile_stride : 0;
     O.image = d_image; O.status = d_status; O.nsteps = d_nsteps;
+    if (O.ntiles == 0) return RAPTOR_OK;
     return run_rays(ctx, O, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int raptor_set_shard(raptor_ctx* ctx, int32_t rank, int32_t world) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (world < 1 || rank < 0 || rank >= world) return fail(ctx, RAPTOR_EINVAL, "shard: need 0 <= rank < world");
+    ctx->shard_rank = rank; ctx->shard_world = world;
+    return RAPTOR_OK;
 }
 
 extern "C" int raptor_flux(raptor_ctx* ctx, const double* d_image, double* d_flux_jy, void* cuda_stream) {

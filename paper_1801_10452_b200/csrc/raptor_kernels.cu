@@ -62,29 +62,30 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         Geom Gs;
         // stage 2 at X + C1x/2, K + C1k/2
         k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-        geom_eval<H1>(P, fma(hl, K[1], X[1]), fma(hl, K[2], X[2]), Gs);
+        geom_shift<H1>(P, G, X[1], X[2], hl * K[1], hl * K[2], Gs);
         geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
         a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
         b0 = fma(2.0, k0, b0); b1 = fma(2.0, k1, b1); b2 = fma(2.0, k2, b2); b3 = fma(2.0, k3, b3);
         // stage 3 at X + C2x/2, K + C2k/2   (C2x = dl * stage-2 wavevector)
         {
-            const double x1s = fma(hl, k1, X[1]), x2s = fma(hl, k2, X[2]);
+            const double d1 = hl * k1, d2 = hl * k2;
             k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-            geom_eval<H1>(P, x1s, x2s, Gs);
+            geom_shift<H1>(P, G, X[1], X[2], d1, d2, Gs);
         }
         geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
         a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
         b0 = fma(2.0, k0, b0); b1 = fma(2.0, k1, b1); b2 = fma(2.0, k2, b2); b3 = fma(2.0, k3, b3);
         // stage 4 at X + C3x, K + C3k
         {
-            const double x1s = fma(dl, k1, X[1]), x2s = fma(dl, k2, X[2]);
+            const double d1 = dl * k1, d2 = dl * k2;
             k0 = fma(dl, f0, K[0]); k1 = fma(dl, f1, K[1]); k2 = fma(dl, f2, K[2]); k3 = fma(dl, f3, K[3]);
-            geom_eval<H1>(P, x1s, x2s, Gs);
+            geom_shift<H1>(P, G, X[1], X[2], d1, d2, Gs);
         }
         geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
         a0 += f0; a1 += f1; a2 += f2; a3 += f3;
         b0 += k0; b1 += k1; b2 += k2; b3 += k3;
         const double d6 = dl * (1.0 / 6.0);
+        const double x1_old = X[1], x2_old = X[2];
         X[0] = fma(d6, b0, X[0]); X[1] = fma(d6, b1, X[1]); X[2] = fma(d6, b2, X[2]); X[3] = fma(d6, b3, X[3]);   // Eq. 15
         K[0] = fma(d6, a0, K[0]); K[1] = fma(d6, a1, K[1]); K[2] = fma(d6, a2, K[2]); K[3] = fma(d6, a3, K[3]);   // Eq. 16
         ++n;
@@ -92,7 +93,10 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
                    is_finite_bits(K[0]) & is_finite_bits(K[1]) & is_finite_bits(K[2]) & is_finite_bits(K[3]);
         if (!fin) { st = S_NONFINITE; break; }
         // ---- new point: geometry shared by transfer, termination, step rule and the next stage 1 ----
-        geom_eval<H1>(P, X[1], X[2], G);
+        // incremental from the old base; re-evaluated from scratch every 16th step so that the round-off of
+        // the increments cannot accumulate (n is warp-uniform: all lanes of a tile start together)
+        if ((n & 15) == 0) geom_eval<H1>(P, X[1], X[2], G);
+        else { Gs = G; geom_shift<H1>(P, Gs, x1_old, x2_old, d6 * b1, d6 * b2, G); }
         if (MODEL != M_VACUUM && G.r >= P.r_in && G.r <= P.r_out) {            // [A8] end-point sample
             Plasma pl;
             if (plasma_sample<MODEL>(P, G, X, K[0], G.ex * K[1], G.dth * K[2], K[3], pl)) {
@@ -133,6 +137,7 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
         if (lane == 0) tile = atomicAdd(O.queue, 1u);
         tile = __shfl_sync(0xffffffffu, tile, 0);
         if (tile >= O.ntiles) break;
+        tile = O.tile_offset + tile * O.tile_stride;                           // multi-GPU shard: interleaved tiles
         double alpha, beta;
         long long pix;
         bool active;

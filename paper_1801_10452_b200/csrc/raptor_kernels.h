@@ -10,7 +10,8 @@ namespace raptor {
 // Outputs and work queue of one launch of the ray kernel.  All pointers are device pointers; any output may be NULL.
 struct RenderOut {
     unsigned int* queue;            // tile counter, zeroed before the launch
-    unsigned int ntiles;
+    unsigned int ntiles;            // tiles this launch processes: global tile = tile_offset + i * tile_stride
+    unsigned int tile_offset, tile_stride;
     unsigned long long* counters;   // [3] steps, sampled steps, rays (accumulated)
     const double* alpha;            // trace mode: explicit impact parameters [nrays]; NULL = render the pixel grid
     const double* beta;
