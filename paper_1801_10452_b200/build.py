@@ -1,17 +1,24 @@
-"""Build of the C-ABI shared library ``libraptor_b200.so`` (in-tree, next to this file) with nvcc for sm_100a."""
+"""Build of the C-ABI shared library ``libraptor_b200.so`` (in-tree, next to this file) with nvcc for sm_100a.
+
+The ray kernel (csrc/raptor_render.cu) is compiled once per plasma model (-DRAPTOR_MODEL=0..5) in parallel;
+objects go to ``build/`` (git-ignored) and are linked with the API and the satellite kernels.
+"""
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libraptor_b200.so")
-SOURCES = ["raptor_kernels.cu", "raptor_api.cu"]
+N_MODELS = 6
 HEADERS = ["raptor_device.cuh", "raptor_kernels.h", os.path.join("..", "..", "include", "raptor.h")]
+SOURCES = ["raptor_render.cu", "raptor_kernels.cu", "raptor_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "--fmad=true", "-Xcompiler", "-fPIC", "-shared"]
+              "--fmad=true", "-Xcompiler", "-fPIC"]
 
 
 def needs_build() -> bool:
@@ -22,14 +29,28 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, extra: list[str] | None = None) -> str:
-    if not force and not needs_build():
-        return LIB
+def build(force: bool = False, verbose: bool = False, extra: list[str] | None = None, out: str | None = None) -> str:
+    """Compiles and links the library; ``extra`` = additional nvcc flags (e.g. -DRAPTOR_MIN_BLOCKS=4),
+    ``out`` = alternative output path."""
+    lib = out or LIB
+    if not force and out is None and not needs_build():
+        return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + (extra or []) + \
-          ["-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
-    subprocess.check_call(cmd)
-    return LIB
+    tag = os.path.splitext(os.path.basename(lib))[0]
+    objdir = os.path.join(OBJ, tag)
+    os.makedirs(objdir, exist_ok=True)
+    base = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + (extra or [])
+    jobs = []
+    for m in range(N_MODELS):
+        o = os.path.join(objdir, f"raptor_render_m{m}.o")
+        jobs.append((base + [f"-DRAPTOR_MODEL={m}", "-c", os.path.join(CSRC, "raptor_render.cu"), "-o", o], o))
+    for src in ("raptor_kernels.cu", "raptor_api.cu"):
+        o = os.path.join(objdir, src.replace(".cu", ".o"))
+        jobs.append((base + ["-c", os.path.join(CSRC, src), "-o", o], o))
+    with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 1)) as pool:
+        list(pool.map(lambda j: subprocess.check_call(j[0]), jobs))
+    subprocess.check_call([nvcc, "-shared", "-o", lib] + [j[1] for j in jobs])
+    return lib
 
 
 if __name__ == "__main__":

@@ -122,7 +122,7 @@ static void build_kp(raptor_ctx* c) {
     const raptor_params& p = c->p;
     KP& k = c->kp;
     std::memset(&k, 0, sizeof(k));
-    k.a = p.a; k.a2 = p.a * p.a; k.m = p.mass; k.omh = 1.0 - p.mks_h; k.r0 = p.mks_r0;
+    k.a = p.a; k.a2 = p.a * p.a; k.twoa = 2.0 * p.a; k.m = p.mass; k.twom = 2.0 * p.mass; k.omh = 1.0 - p.mks_h; k.r0 = p.mks_r0;
     const double inc = p.incl_deg * (kPI / 180.0);
     k.r_cam = p.r_cam; k.sin_i = std::sin(inc); k.cos_i = std::cos(inc);
     k.sq1mc2 = std::sqrt(1.0 - k.cos_i * k.cos_i);

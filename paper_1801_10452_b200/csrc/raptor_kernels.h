@@ -5,6 +5,14 @@
 
 #include "raptor_device.cuh"
 
+// launch shape of the persistent ray kernel: RAPTOR_BLOCK threads per CTA, RAPTOR_MIN_BLOCKS resident CTAs per SM
+#ifndef RAPTOR_BLOCK
+#define RAPTOR_BLOCK 128
+#endif
+#ifndef RAPTOR_MIN_BLOCKS
+#define RAPTOR_MIN_BLOCKS 3
+#endif
+
 namespace raptor {
 
 // Outputs and work queue of one launch of the ray kernel.  All pointers are device pointers; any output may be NULL.
@@ -23,6 +31,9 @@ struct RenderOut {
     double* XK;                     // [npix][8] final state
 };
 
+// raptor_render.cu: one explicit instantiation per plasma model (one translation unit each)
+template <int MODEL>
+cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, cudaStream_t s);
 cudaError_t launch_render(const KP& P, int model, const RenderOut& O, int sm_count, cudaStream_t stream);
 int flux_chunks(size_t npix);
 cudaError_t launch_flux(const double* d_image, size_t npix, int n_freq, double scale, double* d_partial,

@@ -1,0 +1,248 @@
+// raptor_render.cu -- the fused geodesic + radiative-transfer kernel k_render (sm_100a, FP64).
+//
+// Design: one ray per thread with the whole state in registers; persistent
+// warps pull 8x4-pixel tiles from a global atomic counter (work queue at warp granularity: a warp's
+// 32 rays are image neighbours, so they stay in lock-step through vacuum / plasma and end within a
+// few steps of each other, while the queue absorbs the 2x spread in ray length between tiles);
+// the geometry of a point (exp, sincos) is evaluated once and shared by the transfer update, the
+// termination test, the step rule and RK4 stage 1; multi-frequency I/tau live in shared memory.
+//
+// Compiled once per plasma model (-DRAPTOR_MODEL=0..5, in parallel, see build.py) or, without the
+// macro, for all six models in one translation unit.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "raptor_device.cuh"
+#include "raptor_kernels.h"
+
+namespace raptor {
+
+#ifndef RAPTOR_REFRESH
+#define RAPTOR_REFRESH 15      // library exp / sincos at the base point every (RAPTOR_REFRESH + 1)-th step
+#endif
+
+// --------------------------------------------------------------------------------------------
+// One ray (O4 of DESIGN.md).  I/tau access is abstracted: registers (single frequency) or shared memory.
+// FULLX: also integrate X^t and X^phi (needed by the 3-D / slow-light sampler and by the trace output);
+// the metric does not depend on them, so for the other models they are dead and are not computed.
+//
+// RK4, Eq. 7-16, with y = (X, K), y' = (K, f(X, K)), step dl = -h [A2]:
+//   stage wavevectors  k_2 = K + dl/2 f_1,  k_3 = K + dl/2 f_2,  k_4 = K + dl f_3
+//   stage points       X + dl/2 K,  X + dl/2 k_2,  X + dl k_3
+//   X' = X + dl/6 (K + 2 k_2 + 2 k_3 + k_4) = X + dl (K + dl/6 (f_1 + f_2 + f_3))
+//   K' = K + dl/6 (f_1 + 2 f_2 + 2 f_3 + f_4)
+// Only (x1, x2) enter f.  Their exp / sin / cos come incrementally (raptor_device.cuh): stage 2 and stage 4
+// from the base point, stage 3 from stage 2 (offset (dl/2)^2 f_1) and the new base point from stage 4
+// (offset dl^2/6 (f_1 - 2 f_2 + f_3)), both of which are second / third order small.
+// --------------------------------------------------------------------------------------------
+template <int MODEL, bool H1, bool MULTI, bool FULLX>
+__device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta, double* __restrict__ sI,
+                                          double* __restrict__ sTau, int sstride, double& I0, double& tau0,
+                                          double X[4], double K[4], int& status, int& nsteps, int& nsampled) {
+    camera_ray(P, alpha, beta, X, K);
+    double I = 0.0, tau = 0.0;
+    if (MULTI) {
+        for (int k = 0; k < P.n_freq; ++k) { sI[k * sstride] = 0.0; sTau[k * sstride] = 0.0; }
+    }
+    int n = 0, ns = 0, st = S_RUNNING;
+    Geom G;
+    geom_eval<H1>(P, X[1], X[2], G);
+    for (;;) {
+        if (G.r < P.r_in) { st = S_CAPTURED; break; }                         // [A7]
+        if (G.r > P.r_out) { st = S_ESCAPED; break; }
+        if (n >= P.max_steps) { st = S_MAXSTEPS; break; }
+        if (P.use_tau_cutoff) {
+            double tmin = tau;
+            if (MULTI) {
+                tmin = sTau[0];
+                for (int k = 1; k < P.n_freq; ++k) tmin = fmin(tmin, sTau[k * sstride]);
+            }
+            if (tmin > P.tau_cutoff) { st = S_THICK; break; }
+        }
+        const double h = step_size(P, G, X[2], K[1], K[2], K[3]);
+        const double dl = -h;                                                  // backward [A2]
+        const double hl = 0.5 * dl;
+        double f0, f1, f2, f3;          // stage acceleration
+        double k0, k1, k2, k3;          // stage wavevector
+        double a0, a1, a2, a3;          // f_1 + 2 f_2 + 2 f_3 + f_4
+        double s0 = 0.0, s1, s2, s3 = 0.0;   // f_1 + f_2 + f_3   (components t, phi only with FULLX)
+        Geom Gs, Gt;
+        // stage 1 at (X, K)
+        geodesic_rhs(P, G, K[0], K[1], K[2], K[3], f0, f1, f2, f3);
+        a0 = f0; a1 = f1; a2 = f2; a3 = f3;
+        // stage 2 at X + dl/2 K, K + dl/2 f_1
+        k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
+        const double hh = hl * hl;
+        const double e1 = hh * f1, e2 = hh * f2;                               // stage-3 point minus stage-2 point
+        {
+            const double d1 = hl * K[1], d2 = hl * K[2];
+            geom_shift<H1>(P, G, X[1] + d1, X[2] + d2, d1, d2, Gs);
+        }
+        const double x1s3 = fma(hl, k1, X[1]), x2s3 = fma(hl, k2, X[2]);       // stage-3 point (library fallback only)
+        geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
+        if (FULLX) { s0 = a0 + f0; s3 = a3 + f3; }
+        s1 = a1 + f1; s2 = a2 + f2;
+        a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
+        const double g1 = hl * f1, g2 = hl * f2;                               // dl/2 f_2 (x1, x2): end-point offset below
+        // stage 3 at X + dl/2 k_2, K + dl/2 f_2
+        k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
+        geom_shift<H1>(P, Gs, x1s3, x2s3, e1, e2, Gt);
+        geodesic_rhs(P, Gt, k0, k1, k2, k3, f0, f1, f2, f3);
+        if (FULLX) { s0 += f0; s3 += f3; }
+        s1 += f1; s2 += f2;
+        a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
+        // stage 4 at X + dl k_3, K + dl f_3
+        {
+            const double d1 = dl * k1, d2 = dl * k2;
+            geom_shift<H1>(P, G, X[1] + d1, X[2] + d2, d1, d2, Gs);
+        }
+        k0 = fma(dl, f0, K[0]); k1 = fma(dl, f1, K[1]); k2 = fma(dl, f2, K[2]); k3 = fma(dl, f3, K[3]);
+        geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
+        a0 += f0; a1 += f1; a2 += f2; a3 += f3;
+        const double d6 = dl * (1.0 / 6.0);
+        // new point minus stage-4 point: dl (K + dl/6 S) - dl k_3 = dl (dl/6 S - dl/2 f_2)
+        const double t1 = dl * fma(d6, s1, -g1), t2 = dl * fma(d6, s2, -g2);
+        if (FULLX) { X[0] = fma(dl, fma(d6, s0, K[0]), X[0]); X[3] = fma(dl, fma(d6, s3, K[3]), X[3]); }     // Eq. 15
+        X[1] = fma(dl, fma(d6, s1, K[1]), X[1]); X[2] = fma(dl, fma(d6, s2, K[2]), X[2]);
+        K[0] = fma(d6, a0, K[0]); K[1] = fma(d6, a1, K[1]); K[2] = fma(d6, a2, K[2]); K[3] = fma(d6, a3, K[3]);   // Eq. 16
+        ++n;
+        bool fin = is_finite_bits(X[1]) & is_finite_bits(X[2]) &
+                   is_finite_bits(K[0]) & is_finite_bits(K[1]) & is_finite_bits(K[2]) & is_finite_bits(K[3]);
+        if (FULLX) fin = fin & is_finite_bits(X[0]) & is_finite_bits(X[3]);
+        if (!fin) { st = S_NONFINITE; break; }
+        // ---- new point: geometry shared by transfer, termination, step rule and the next stage 1 ----
+        // incremental from stage 4; re-evaluated with the library functions every (RAPTOR_REFRESH+1)-th step so
+        // that the round-off of the increments cannot accumulate (n is warp-uniform: a tile's lanes start together)
+        if ((n & RAPTOR_REFRESH) == 0) geom_eval<H1>(P, X[1], X[2], G);
+        else geom_shift<H1>(P, Gs, X[1], X[2], t1, t2, G);
+        if (MODEL != M_VACUUM && G.r >= P.r_in && G.r <= P.r_out) {            // [A8] end-point sample
+            Plasma pl;
+            if (plasma_sample<MODEL>(P, G, X, K[0], G.ex * K[1], G.dth * K[2], K[3], pl)) {
+                ++ns;
+                EmisConst E;
+                emis_prepare(P, pl, h, E);
+                if (MULTI) {
+                    for (int k = 0; k < P.n_freq; ++k) {
+                        double Ik = sI[k * sstride], tk = sTau[k * sstride];
+                        transfer_one(pl, E, __ldg(P.freq + k), Ik, tk);
+                        sI[k * sstride] = Ik; sTau[k * sstride] = tk;
+                    }
+                } else {
+                    transfer_one(pl, E, __ldg(P.freq), I, tau);
+                }
+            }
+        }
+    }
+    I0 = I; tau0 = tau;
+    status = st; nsteps = n; nsampled = ns;
+}
+
+// --------------------------------------------------------------------------------------------
+// Persistent-warp driver: tiles of 8x4 pixels (render) or 32 consecutive rays (trace) from a global queue.
+// --------------------------------------------------------------------------------------------
+template <int MODEL, bool H1, bool MULTI, bool FULLX>
+__global__ void __launch_bounds__(RAPTOR_BLOCK, RAPTOR_MIN_BLOCKS)
+k_render(const __grid_constant__ KP P, const RenderOut O) {
+    extern __shared__ double smem[];
+    const int lane = threadIdx.x & 31;
+    double* sI = MULTI ? smem + threadIdx.x : nullptr;                         // [k][thread]: conflict-free
+    double* sTau = MULTI ? smem + (size_t)P.n_freq * blockDim.x + threadIdx.x : nullptr;
+    const int sstride = blockDim.x;
+    const int ntx = (P.nx + 7) >> 3;
+    unsigned long long steps = 0, sampled = 0, rays = 0;
+    for (;;) {
+        unsigned int tile = 0;
+        if (lane == 0) tile = atomicAdd(O.queue, 1u);
+        tile = __shfl_sync(0xffffffffu, tile, 0);
+        if (tile >= O.ntiles) break;
+        tile = O.tile_offset + tile * O.tile_stride;                           // multi-GPU shard: interleaved tiles
+        double alpha, beta;
+        long long pix;
+        bool active;
+        if (O.alpha) {                                                         // trace mode: explicit impact parameters
+            pix = (long long)tile * 32 + lane;
+            active = pix < O.nrays;
+            alpha = active ? O.alpha[pix] : 0.0;
+            beta = active ? O.beta[pix] : 0.0;
+        } else {
+            const int ty = tile / ntx, tx = tile - ty * ntx;
+            const int ix = (tx << 3) + (lane & 7), iy = (ty << 2) + (lane >> 3);
+            active = ix < P.nx && iy < P.ny;
+            alpha = fma((double)ix + 0.5, P.pix_dx, -0.5 * P.fov);             // pixel centres [A4b]
+            beta = fma((double)iy + 0.5, P.pix_dy, -0.5 * P.fov);
+            pix = (long long)iy * P.nx + ix;
+        }
+        if (active) {
+            double X[4], K[4], I0, tau0;
+            int status, n, ns;
+            trace_ray<MODEL, H1, MULTI, FULLX>(P, alpha, beta, sI, sTau, sstride, I0, tau0, X, K, status, n, ns);
+            steps += (unsigned)n; sampled += (unsigned)ns; rays += 1;
+            const size_t npix = O.alpha ? (size_t)O.nrays : (size_t)P.nx * P.ny;
+            if (O.image) {
+                if (MULTI) { for (int k = 0; k < P.n_freq; ++k) O.image[(size_t)k * npix + pix] = sI[k * sstride]; }
+                else O.image[pix] = I0;
+            }
+            if (O.tau) {
+                if (MULTI) { for (int k = 0; k < P.n_freq; ++k) O.tau[(size_t)k * npix + pix] = sTau[k * sstride]; }
+                else O.tau[pix] = tau0;
+            }
+            if (O.status) O.status[pix] = status;
+            if (O.nsteps) O.nsteps[pix] = n;
+            if (FULLX && O.XK) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) { O.XK[pix * 8 + i] = X[i]; O.XK[pix * 8 + 4 + i] = K[i]; }
+            }
+        }
+        __syncwarp();
+    }
+    // counters: warp reduce, one atomic per warp
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        steps += __shfl_down_sync(0xffffffffu, steps, o);
+        sampled += __shfl_down_sync(0xffffffffu, sampled, o);
+        rays += __shfl_down_sync(0xffffffffu, rays, o);
+    }
+    if (lane == 0) {
+        atomicAdd(O.counters + 0, steps);
+        atomicAdd(O.counters + 1, sampled);
+        atomicAdd(O.counters + 2, rays);
+    }
+}
+
+template <int MODEL, bool H1, bool MULTI, bool FULLX>
+static cudaError_t launch_one(const KP& P, const RenderOut& O, int grid, cudaStream_t stream) {
+    size_t smem = MULTI ? (size_t)2 * P.n_freq * RAPTOR_BLOCK * sizeof(double) : 0;
+    auto kern = k_render<MODEL, H1, MULTI, FULLX>;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    kern<<<grid, RAPTOR_BLOCK, smem, stream>>>(P, O);
+    return cudaGetLastError();
+}
+
+template <int MODEL, bool FULLX>
+static cudaError_t launch_hm(const KP& P, const RenderOut& O, bool h1, bool multi, int grid, cudaStream_t s) {
+    if (h1) return multi ? launch_one<MODEL, true, true, FULLX>(P, O, grid, s) : launch_one<MODEL, true, false, FULLX>(P, O, grid, s);
+    return multi ? launch_one<MODEL, false, true, FULLX>(P, O, grid, s) : launch_one<MODEL, false, false, FULLX>(P, O, grid, s);
+}
+
+template <int MODEL>
+cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, cudaStream_t s) {
+    // the 3-D / slow-light sampler reads X^t, X^phi: always FULLX; the other models need them for the XK output only
+    if (MODEL == M_GRID3DT || fullx) return launch_hm<MODEL, true>(P, O, h1, multi, grid, s);
+    return launch_hm<MODEL, MODEL == M_GRID3DT>(P, O, h1, multi, grid, s);
+}
+
+#ifdef RAPTOR_MODEL
+template cudaError_t launch_model<RAPTOR_MODEL>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+#else
+template cudaError_t launch_model<M_VACUUM>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+template cudaError_t launch_model<M_SPHERE>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+template cudaError_t launch_model<M_TORUS>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+template cudaError_t launch_model<M_GRID2D>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+template cudaError_t launch_model<M_GRID3DT>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+template cudaError_t launch_model<M_SLAB>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+#endif
+
+}  // namespace raptor
