@@ -10,7 +10,7 @@
 #define RAPTOR_BLOCK 128
 #endif
 #ifndef RAPTOR_MIN_BLOCKS
-#define RAPTOR_MIN_BLOCKS 3
+#define RAPTOR_MIN_BLOCKS 4
 #endif
 
 namespace raptor {

@@ -46,7 +46,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
     }
     int n = 0, ns = 0, st = S_RUNNING;
     Geom G;
-    geom_eval<H1>(P, X[1], X[2], G);
+    { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
     for (;;) {
         if (G.r < P.r_in) { st = S_CAPTURED; break; }                         // [A7]
         if (G.r > P.r_out) { st = S_ESCAPED; break; }
@@ -113,7 +113,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         // ---- new point: geometry shared by transfer, termination, step rule and the next stage 1 ----
         // incremental from stage 4; re-evaluated with the library functions every (RAPTOR_REFRESH+1)-th step so
         // that the round-off of the increments cannot accumulate (n is warp-uniform: a tile's lanes start together)
-        if ((n & RAPTOR_REFRESH) == 0) geom_eval<H1>(P, X[1], X[2], G);
+        if ((n & RAPTOR_REFRESH) == 0) { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
         else geom_shift<H1>(P, Gs, X[1], X[2], t1, t2, G);
         if (MODEL != M_VACUUM && G.r >= P.r_in && G.r <= P.r_out) {            // [A8] end-point sample
             Plasma pl;
