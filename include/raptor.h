@@ -59,7 +59,9 @@ typedef struct {
     double M_bh_g;             /* black-hole mass [g]: L = G M / c^2 */
     double D_src_cm;           /* distance [cm] */
     double M_unit_g;           /* mass unit [g]: rho0 = M_unit / L^3 (grid models) */
-    /* integrator: RK4, Eq. 7-16, backward (d lambda = -h) [A2] */
+    /* integrator (field `integrator` below), backward (d lambda = -h) [A2]: RK4 Eq. 7-16;
+     * velocity Verlet Eq. 17-20 without / with the corrector re-evaluation of PAPER.md:127;
+     * "RK2" of Table B.1 = explicit midpoint [A17] */
     double step_c, step_min, step_max;   /* policy A: h = clamp(c (r - r_H), min, max) (BASELINE.json configs[0]) */
     double eps, delta;         /* policy B: Eq. 21-24 */
     double eps_polar;          /* policy A polar guard: h <= eps_polar r |sin theta| (Eq. 23 with |k^theta| <= 1/r) */
@@ -78,7 +80,7 @@ typedef struct {
     const void *grid_host;     /* host, AoS [nt][n1][n2][n3][8] = rho, u, u~1, u~2, u~3, B1, B2, B3 (HARM primitives) */
     uint64_t grid_bytes;       /* must equal nt*n1*n2*n3*8*sizeof(element) */
     int32_t nx, ny;            /* pixels */
-    int32_t integrator;        /* 0 = RK4 */
+    int32_t integrator;        /* 0 = RK4, 1 = Verlet, 2 = Verlet + corrector, 3 = RK2 (midpoint) */
     int32_t step_policy;       /* 0 = A, 1 = B */
     int32_t max_steps;         /* per ray */
     int32_t n_freq;            /* 1 .. RAPTOR_MAX_FREQ */

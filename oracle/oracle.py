@@ -83,6 +83,9 @@ def lib():
         _lib.orc_metric_ks_inv.argtypes = [C.c_double] * 4 + [_D44]
         _lib.orc_camera_ab.argtypes = [C.POINTER(OrcParams), C.c_double, C.c_double, _D4, _D4]
         _lib.orc_rk4_step.argtypes = [C.POINTER(OrcParams), _D4, _D4, C.c_double]
+        _lib.orc_verlet_step.argtypes = [C.POINTER(OrcParams), _D4, _D4, C.c_double, C.c_int]
+        _lib.orc_rk2_step.argtypes = [C.POINTER(OrcParams), _D4, _D4, C.c_double]
+        _lib.orc_step.argtypes = [C.POINTER(OrcParams), _D4, _D4, C.c_double]
         _lib.orc_trace_ray.argtypes = [C.POINTER(OrcParams), C.c_double, C.c_double, C.c_void_p, C.c_void_p,
                                        C.POINTER(RayResult), C.c_void_p, C.c_int, C.c_int]
     return _lib
@@ -171,6 +174,22 @@ class Oracle:
     def rk4_step(self, X, K, dl):
         Xc, Kc = _D4(*X), _D4(*K)
         self.lib.orc_rk4_step(C.byref(self.p), Xc, Kc, float(dl))
+        return np.array(Xc), np.array(Kc)
+
+    def verlet_step(self, X, K, dl, corrector=False):
+        Xc, Kc = _D4(*X), _D4(*K)
+        self.lib.orc_verlet_step(C.byref(self.p), Xc, Kc, float(dl), 1 if corrector else 0)
+        return np.array(Xc), np.array(Kc)
+
+    def rk2_step(self, X, K, dl):
+        Xc, Kc = _D4(*X), _D4(*K)
+        self.lib.orc_rk2_step(C.byref(self.p), Xc, Kc, float(dl))
+        return np.array(Xc), np.array(Kc)
+
+    def step(self, X, K, dl):
+        """One step of the scene's integrator (0 RK4, 1 Verlet, 2 Verlet + corrector, 3 RK2)."""
+        Xc, Kc = _D4(*X), _D4(*K)
+        self.lib.orc_step(C.byref(self.p), Xc, Kc, float(dl))
         return np.array(Xc), np.array(Kc)
 
     # ---- plasma + transfer ----------------------------------------------------------

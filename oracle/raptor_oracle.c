@@ -356,6 +356,50 @@ void orc_rk4_step(const orc_params *P, double X[4], double K[4], double dl)
  * stage is dl times the STAGE wavevector, i.e. k + C_{1,k}/2 -- with C_{1,x} the printed form
  * would add a length to a wavevector.  Read as the k-coefficient [A21 in DESIGN.md]. */
 
+/* Velocity Verlet, Eq. 17-20.  (dk/dl)_n is evaluated from the current (x_n, k_n) at the
+ * start of every step [A23 in DESIGN.md]: the scheme is then a map of (x_n, k_n) alone, and the paper's cost
+ * argument (fewer evaluations of the connection) is unaffected because the connection at x_n was
+ * already evaluated by the previous step's Eq. 19.  corrector != 0 adds the refinement of PAPER.md:127: Eq. 19
+ * re-evaluated with k_{n+1,p} = k_{n+1}, then Eq. 20 again. */
+void orc_verlet_step(const orc_params *P, double X[4], double K[4], double dl, int corrector)
+{
+    double fn[4], fn1[4], Xn[4], Kp[4], Kn[4];
+    int i;
+    orc_rhs(P, X, K, fn);
+    for (i = 0; i < 4; ++i) Xn[i] = X[i] + K[i] * dl + 0.5 * fn[i] * (dl * dl);              /* 17 */
+    for (i = 0; i < 4; ++i) Kp[i] = K[i] + fn[i] * dl;                                       /* 18 */
+    orc_rhs(P, Xn, Kp, fn1);                                                                 /* 19 */
+    for (i = 0; i < 4; ++i) Kn[i] = K[i] + 0.5 * (fn[i] + fn1[i]) * dl;                      /* 20 */
+    if (corrector) {
+        orc_rhs(P, Xn, Kn, fn1);                                                             /* 19 with k_{n+1} */
+        for (i = 0; i < 4; ++i) Kn[i] = K[i] + 0.5 * (fn[i] + fn1[i]) * dl;                  /* 20 again */
+    }
+    for (i = 0; i < 4; ++i) { X[i] = Xn[i]; K[i] = Kn[i]; }
+}
+
+/* "RK2": Table B.1 names it, the paper never defines it.  Read as the explicit midpoint
+ * method, the two-stage member of the family Eq. 7-16 belong to [A17]. */
+void orc_rk2_step(const orc_params *P, double X[4], double K[4], double dl)
+{
+    double f[4], Xs[4], Ks[4];
+    int i;
+    orc_rhs(P, X, K, f);
+    for (i = 0; i < 4; ++i) { Xs[i] = X[i] + 0.5 * dl * K[i]; Ks[i] = K[i] + 0.5 * dl * f[i]; }
+    orc_rhs(P, Xs, Ks, f);
+    for (i = 0; i < 4; ++i) { X[i] = X[i] + dl * Ks[i]; K[i] = K[i] + dl * f[i]; }
+}
+
+/* integrator: 0 = RK4 (Eq. 7-16), 1 = Verlet (Eq. 17-20), 2 = Verlet + corrector, 3 = RK2 [A17] */
+void orc_step(const orc_params *P, double X[4], double K[4], double dl)
+{
+    switch (P->integrator) {
+        case 1: orc_verlet_step(P, X, K, dl, 0); break;
+        case 2: orc_verlet_step(P, X, K, dl, 1); break;
+        case 3: orc_rk2_step(P, X, K, dl); break;
+        default: orc_rk4_step(P, X, K, dl); break;
+    }
+}
+
 /* ======================================================================================= */
 /* Grid interpolation [A16] / O6                                                             */
 /* ======================================================================================= */
@@ -630,7 +674,7 @@ void orc_trace_ray(const orc_params *P, double alpha, double beta, double *I, do
             if (tmin > P->tau_cutoff) { status = ORC_THICK; break; }
         }
         double h = orc_step_size(P, X, K);
-        orc_rk4_step(P, X, K, -h);                                             /* backward [A2] */
+        orc_step(P, X, K, -h);                                                 /* backward [A2] */
         ++n;
         int fin = 1;
         for (int i = 0; i < 4; ++i) if (!isfinite(X[i]) || !isfinite(K[i])) fin = 0;

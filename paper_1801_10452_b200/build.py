@@ -1,6 +1,7 @@
 """Build of the C-ABI shared library ``libraptor_b200.so`` (in-tree, next to this file) with nvcc for sm_100a.
 
-The ray kernel (csrc/raptor_render.cu) is compiled once per plasma model (-DRAPTOR_MODEL=0..5) in parallel;
+The ray kernel (csrc/raptor_render.cu) is compiled once per (plasma model, integrator)
+(-DRAPTOR_MODEL=0..5 -DRAPTOR_INTEG=0..3) in parallel;
 objects go to ``build/`` (git-ignored) and are linked with the API and the satellite kernels.
 """
 from __future__ import annotations
@@ -15,6 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libraptor_b200.so")
 N_MODELS = 6
+N_INTEG = 4
 HEADERS = ["raptor_device.cuh", "raptor_kernels.h", os.path.join("..", "..", "include", "raptor.h")]
 SOURCES = ["raptor_render.cu", "raptor_kernels.cu", "raptor_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -42,14 +44,16 @@ def build(force: bool = False, verbose: bool = False, extra: list[str] | None = 
     base = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + (extra or [])
     jobs = []
     for m in range(N_MODELS):
-        o = os.path.join(objdir, f"raptor_render_m{m}.o")
-        jobs.append((base + [f"-DRAPTOR_MODEL={m}", "-c", os.path.join(CSRC, "raptor_render.cu"), "-o", o], o))
+        for i in range(N_INTEG):
+            o = os.path.join(objdir, f"raptor_render_m{m}_i{i}.o")
+            jobs.append((base + [f"-DRAPTOR_MODEL={m}", f"-DRAPTOR_INTEG={i}", "-c",
+                                 os.path.join(CSRC, "raptor_render.cu"), "-o", o], o))
     for src in ("raptor_kernels.cu", "raptor_api.cu"):
         o = os.path.join(objdir, src.replace(".cu", ".o"))
         jobs.append((base + ["-c", os.path.join(CSRC, src), "-o", o], o))
     with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 1)) as pool:
         list(pool.map(lambda j: subprocess.check_call(j[0]), jobs))
-    subprocess.check_call([nvcc, "-shared", "-o", lib] + [j[1] for j in jobs])
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", lib] + [j[1] for j in jobs])
     return lib
 
 

@@ -90,7 +90,7 @@ static int validate(const raptor_params* p) {
     if (!(p->r_cam > rH) || !(p->r_cam > p->mks_r0)) return fail(nullptr, RAPTOR_EINVAL, "r_cam must be outside the horizon");
     if (!(p->mks_r0 < rH || p->mass == 0.0)) return fail(nullptr, RAPTOR_EINVAL, "mks_r0 must be < r_H");
     if (!(p->fov_M > 0.0)) return fail(nullptr, RAPTOR_EINVAL, "fov_M must be > 0");
-    if (p->integrator != 0) return fail(nullptr, RAPTOR_EUNSUPPORTED, "integrator %d: only 0 (RK4) is built", p->integrator);
+    if (p->integrator < 0 || p->integrator > 3) return fail(nullptr, RAPTOR_EINVAL, "integrator %d: 0 RK4, 1 Verlet, 2 Verlet + corrector, 3 RK2", p->integrator);
     if (p->step_policy != 0 && p->step_policy != 1) return fail(nullptr, RAPTOR_EINVAL, "step_policy must be 0 or 1");
     if (p->step_policy == 0 && !(p->step_min > 0.0 && p->step_max >= p->step_min && p->step_c >= 0.0 && p->eps_polar > 0.0))
         return fail(nullptr, RAPTOR_EINVAL, "policy A needs 0 < step_min <= step_max, step_c >= 0, eps_polar > 0");
@@ -149,7 +149,7 @@ static void build_kp(raptor_ctx* c) {
     }
     k.t0 = p.t0; k.inv_dt = p.dt_snap > 0.0 ? 1.0 / p.dt_snap : 0.0;
     k.grid = c->d_grid; k.freq = c->d_freq;
-    k.nx = p.nx; k.ny = p.ny; k.step_policy = p.step_policy; k.max_steps = p.max_steps; k.n_freq = p.n_freq;
+    k.nx = p.nx; k.ny = p.ny; k.integrator = p.integrator; k.step_policy = p.step_policy; k.max_steps = p.max_steps; k.n_freq = p.n_freq;
     k.k2_mode = p.k2_mode; k.n1 = p.n1; k.n2 = p.n2; k.n3 = p.n3; k.nt = p.nt;
     k.slow_light = p.slow_light; k.snapshot = p.snapshot;
 }

@@ -22,13 +22,16 @@ cudaError_t launch_render(const KP& P, int model, const RenderOut& O, int sm_cou
     int grid = sm_count * per_sm;
     if (want < grid) grid = (int)(want > 0 ? want : 1);
     const bool fullx = O.XK != nullptr;
+#define RAPTOR_CASE_I(M, I) case I: return launch_model<M, I>(P, O, h1, multi, fullx, grid, stream);
+#define RAPTOR_CASE_M(M)                                                                          \
+    case M:                                                                                       \
+        switch (P.integrator) {                                                                   \
+            RAPTOR_CASE_I(M, I_RK4) RAPTOR_CASE_I(M, I_VERLET) RAPTOR_CASE_I(M, I_VERLET_C) RAPTOR_CASE_I(M, I_RK2) \
+        }                                                                                         \
+        break;
     switch (model) {
-        case M_VACUUM: return launch_model<M_VACUUM>(P, O, h1, multi, fullx, grid, stream);
-        case M_SPHERE: return launch_model<M_SPHERE>(P, O, h1, multi, fullx, grid, stream);
-        case M_TORUS: return launch_model<M_TORUS>(P, O, h1, multi, fullx, grid, stream);
-        case M_GRID2D: return launch_model<M_GRID2D>(P, O, h1, multi, fullx, grid, stream);
-        case M_GRID3DT: return launch_model<M_GRID3DT>(P, O, h1, multi, fullx, grid, stream);
-        case M_SLAB: return launch_model<M_SLAB>(P, O, h1, multi, fullx, grid, stream);
+        RAPTOR_CASE_M(M_VACUUM) RAPTOR_CASE_M(M_SPHERE) RAPTOR_CASE_M(M_TORUS)
+        RAPTOR_CASE_M(M_GRID2D) RAPTOR_CASE_M(M_GRID3DT) RAPTOR_CASE_M(M_SLAB)
     }
     return cudaErrorInvalidValue;
 }

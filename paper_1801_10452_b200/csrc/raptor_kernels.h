@@ -31,8 +31,8 @@ struct RenderOut {
     double* XK;                     // [npix][8] final state
 };
 
-// raptor_render.cu: one explicit instantiation per plasma model (one translation unit each)
-template <int MODEL>
+// raptor_render.cu: one explicit instantiation per (plasma model, integrator), one translation unit each
+template <int MODEL, int INTEG>
 cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, cudaStream_t s);
 cudaError_t launch_render(const KP& P, int model, const RenderOut& O, int sm_count, cudaStream_t stream);
 int flux_chunks(size_t npix);

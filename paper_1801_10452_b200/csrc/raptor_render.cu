@@ -35,7 +35,7 @@ namespace raptor {
 // from the base point, stage 3 from stage 2 (offset (dl/2)^2 f_1) and the new base point from stage 4
 // (offset dl^2/6 (f_1 - 2 f_2 + f_3)), both of which are second / third order small.
 // --------------------------------------------------------------------------------------------
-template <int MODEL, bool H1, bool MULTI, bool FULLX>
+template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG>
 __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta, double* __restrict__ sI,
                                           double* __restrict__ sTau, int sstride, double& I0, double& tau0,
                                           double X[4], double K[4], int& status, int& nsteps, int& nsampled) {
@@ -62,49 +62,87 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         const double h = step_size(P, G, X[2], K[1], K[2], K[3]);
         const double dl = -h;                                                  // backward [A2]
         const double hl = 0.5 * dl;
-        double f0, f1, f2, f3;          // stage acceleration
-        double k0, k1, k2, k3;          // stage wavevector
-        double a0, a1, a2, a3;          // f_1 + 2 f_2 + 2 f_3 + f_4
-        double s0 = 0.0, s1, s2, s3 = 0.0;   // f_1 + f_2 + f_3   (components t, phi only with FULLX)
-        Geom Gs, Gt;
-        // stage 1 at (X, K)
-        geodesic_rhs(P, G, K[0], K[1], K[2], K[3], f0, f1, f2, f3);
-        a0 = f0; a1 = f1; a2 = f2; a3 = f3;
-        // stage 2 at X + dl/2 K, K + dl/2 f_1
-        k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-        const double hh = hl * hl;
-        const double e1 = hh * f1, e2 = hh * f2;                               // stage-3 point minus stage-2 point
-        {
+        Geom Gs;                        // geometry of the last stage point: the new base point is reached from it
+        double t1, t2;                  // new point minus that stage point (x1, x2)
+        if (INTEG == I_RK4) {
+            double f0, f1, f2, f3;          // stage acceleration
+            double k0, k1, k2, k3;          // stage wavevector
+            double a0, a1, a2, a3;          // f_1 + 2 f_2 + 2 f_3 + f_4
+            double s0 = 0.0, s1, s2, s3 = 0.0;   // f_1 + f_2 + f_3   (components t, phi only with FULLX)
+            Geom Gt;
+            // stage 1 at (X, K)
+            geodesic_rhs(P, G, K[0], K[1], K[2], K[3], f0, f1, f2, f3);
+            a0 = f0; a1 = f1; a2 = f2; a3 = f3;
+            // stage 2 at X + dl/2 K, K + dl/2 f_1
+            k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
+            const double hh = hl * hl;
+            const double e1 = hh * f1, e2 = hh * f2;                               // stage-3 point minus stage-2 point
+            {
+                const double d1 = hl * K[1], d2 = hl * K[2];
+                geom_shift<H1>(P, G, X[1] + d1, X[2] + d2, d1, d2, Gs);
+            }
+            const double x1s3 = fma(hl, k1, X[1]), x2s3 = fma(hl, k2, X[2]);       // stage-3 point (library fallback only)
+            geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
+            if (FULLX) { s0 = a0 + f0; s3 = a3 + f3; }
+            s1 = a1 + f1; s2 = a2 + f2;
+            a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
+            const double g1 = hl * f1, g2 = hl * f2;                               // dl/2 f_2 (x1, x2): end-point offset below
+            // stage 3 at X + dl/2 k_2, K + dl/2 f_2
+            k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
+            geom_shift<H1>(P, Gs, x1s3, x2s3, e1, e2, Gt);
+            geodesic_rhs(P, Gt, k0, k1, k2, k3, f0, f1, f2, f3);
+            if (FULLX) { s0 += f0; s3 += f3; }
+            s1 += f1; s2 += f2;
+            a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
+            // stage 4 at X + dl k_3, K + dl f_3
+            {
+                const double d1 = dl * k1, d2 = dl * k2;
+                geom_shift<H1>(P, G, X[1] + d1, X[2] + d2, d1, d2, Gs);
+            }
+            k0 = fma(dl, f0, K[0]); k1 = fma(dl, f1, K[1]); k2 = fma(dl, f2, K[2]); k3 = fma(dl, f3, K[3]);
+            geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
+            a0 += f0; a1 += f1; a2 += f2; a3 += f3;
+            const double d6 = dl * (1.0 / 6.0);
+            // new point minus stage-4 point: dl (K + dl/6 S) - dl k_3 = dl (dl/6 S - dl/2 f_2)
+            t1 = dl * fma(d6, s1, -g1); t2 = dl * fma(d6, s2, -g2);
+            if (FULLX) { X[0] = fma(dl, fma(d6, s0, K[0]), X[0]); X[3] = fma(dl, fma(d6, s3, K[3]), X[3]); }     // Eq. 15
+            X[1] = fma(dl, fma(d6, s1, K[1]), X[1]); X[2] = fma(dl, fma(d6, s2, K[2]), X[2]);
+            K[0] = fma(d6, a0, K[0]); K[1] = fma(d6, a1, K[1]); K[2] = fma(d6, a2, K[2]); K[3] = fma(d6, a3, K[3]);   // Eq. 16
+        } else if (INTEG == I_RK2) {
+            // "RK2" of Table B.1, read as the explicit midpoint method [A17]
+            double f0, f1, f2, f3, k0, k1, k2, k3;
+            geodesic_rhs(P, G, K[0], K[1], K[2], K[3], f0, f1, f2, f3);
+            k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
             const double d1 = hl * K[1], d2 = hl * K[2];
             geom_shift<H1>(P, G, X[1] + d1, X[2] + d2, d1, d2, Gs);
+            geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
+            // new point minus midpoint: dl k_mid - dl/2 K
+            t1 = fma(dl, k1, -d1); t2 = fma(dl, k2, -d2);
+            if (FULLX) { X[0] = fma(dl, k0, X[0]); X[3] = fma(dl, k3, X[3]); }
+            X[1] = fma(dl, k1, X[1]); X[2] = fma(dl, k2, X[2]);
+            K[0] = fma(dl, f0, K[0]); K[1] = fma(dl, f1, K[1]); K[2] = fma(dl, f2, K[2]); K[3] = fma(dl, f3, K[3]);
+        } else {
+            // velocity Verlet, Eq. 17-20; (dk/dl)_n from the current (x_n, k_n) [A23];
+            // I_VERLET_C: Eq. 19 re-evaluated with k_{n+1,p} = k_{n+1}, then Eq. 20 again
+            double f0, f1, f2, f3, g0, g1, g2, g3, p0, p1, p2, p3;
+            geodesic_rhs(P, G, K[0], K[1], K[2], K[3], f0, f1, f2, f3);
+            const double hd2 = 0.5 * (dl * dl);
+            t1 = fma(hd2, f1, dl * K[1]); t2 = fma(hd2, f2, dl * K[2]);                        // Eq. 17
+            if (FULLX) { X[0] += fma(hd2, f0, dl * K[0]); X[3] += fma(hd2, f3, dl * K[3]); }
+            X[1] += t1; X[2] += t2;
+            p0 = fma(dl, f0, K[0]); p1 = fma(dl, f1, K[1]); p2 = fma(dl, f2, K[2]); p3 = fma(dl, f3, K[3]);   // Eq. 18
+            geom_shift<H1>(P, G, X[1], X[2], t1, t2, Gs);
+            geodesic_rhs(P, Gs, p0, p1, p2, p3, g0, g1, g2, g3);                                // Eq. 19
+            p0 = fma(hl, f0 + g0, K[0]); p1 = fma(hl, f1 + g1, K[1]);                           // Eq. 20
+            p2 = fma(hl, f2 + g2, K[2]); p3 = fma(hl, f3 + g3, K[3]);
+            if (INTEG == I_VERLET_C) {
+                geodesic_rhs(P, Gs, p0, p1, p2, p3, g0, g1, g2, g3);
+                p0 = fma(hl, f0 + g0, K[0]); p1 = fma(hl, f1 + g1, K[1]);
+                p2 = fma(hl, f2 + g2, K[2]); p3 = fma(hl, f3 + g3, K[3]);
+            }
+            K[0] = p0; K[1] = p1; K[2] = p2; K[3] = p3;
+            t1 = 0.0; t2 = 0.0;                                                                 // Gs is the new point
         }
-        const double x1s3 = fma(hl, k1, X[1]), x2s3 = fma(hl, k2, X[2]);       // stage-3 point (library fallback only)
-        geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
-        if (FULLX) { s0 = a0 + f0; s3 = a3 + f3; }
-        s1 = a1 + f1; s2 = a2 + f2;
-        a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
-        const double g1 = hl * f1, g2 = hl * f2;                               // dl/2 f_2 (x1, x2): end-point offset below
-        // stage 3 at X + dl/2 k_2, K + dl/2 f_2
-        k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-        geom_shift<H1>(P, Gs, x1s3, x2s3, e1, e2, Gt);
-        geodesic_rhs(P, Gt, k0, k1, k2, k3, f0, f1, f2, f3);
-        if (FULLX) { s0 += f0; s3 += f3; }
-        s1 += f1; s2 += f2;
-        a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
-        // stage 4 at X + dl k_3, K + dl f_3
-        {
-            const double d1 = dl * k1, d2 = dl * k2;
-            geom_shift<H1>(P, G, X[1] + d1, X[2] + d2, d1, d2, Gs);
-        }
-        k0 = fma(dl, f0, K[0]); k1 = fma(dl, f1, K[1]); k2 = fma(dl, f2, K[2]); k3 = fma(dl, f3, K[3]);
-        geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
-        a0 += f0; a1 += f1; a2 += f2; a3 += f3;
-        const double d6 = dl * (1.0 / 6.0);
-        // new point minus stage-4 point: dl (K + dl/6 S) - dl k_3 = dl (dl/6 S - dl/2 f_2)
-        const double t1 = dl * fma(d6, s1, -g1), t2 = dl * fma(d6, s2, -g2);
-        if (FULLX) { X[0] = fma(dl, fma(d6, s0, K[0]), X[0]); X[3] = fma(dl, fma(d6, s3, K[3]), X[3]); }     // Eq. 15
-        X[1] = fma(dl, fma(d6, s1, K[1]), X[1]); X[2] = fma(dl, fma(d6, s2, K[2]), X[2]);
-        K[0] = fma(d6, a0, K[0]); K[1] = fma(d6, a1, K[1]); K[2] = fma(d6, a2, K[2]); K[3] = fma(d6, a3, K[3]);   // Eq. 16
         ++n;
         bool fin = is_finite_bits(X[1]) & is_finite_bits(X[2]) &
                    is_finite_bits(K[0]) & is_finite_bits(K[1]) & is_finite_bits(K[2]) & is_finite_bits(K[3]);
@@ -114,6 +152,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         // incremental from stage 4; re-evaluated with the library functions every (RAPTOR_REFRESH+1)-th step so
         // that the round-off of the increments cannot accumulate (n is warp-uniform: a tile's lanes start together)
         if ((n & RAPTOR_REFRESH) == 0) { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
+        else if (INTEG == I_VERLET || INTEG == I_VERLET_C) G = Gs;
         else geom_shift<H1>(P, Gs, X[1], X[2], t1, t2, G);
         if (MODEL != M_VACUUM && G.r >= P.r_in && G.r <= P.r_out) {            // [A8] end-point sample
             Plasma pl;
@@ -140,7 +179,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
 // --------------------------------------------------------------------------------------------
 // Persistent-warp driver: tiles of 8x4 pixels (render) or 32 consecutive rays (trace) from a global queue.
 // --------------------------------------------------------------------------------------------
-template <int MODEL, bool H1, bool MULTI, bool FULLX>
+template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG>
 __global__ void __launch_bounds__(RAPTOR_BLOCK, RAPTOR_MIN_BLOCKS)
 k_render(const __grid_constant__ KP P, const RenderOut O) {
     extern __shared__ double smem[];
@@ -175,7 +214,7 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
         if (active) {
             double X[4], K[4], I0, tau0;
             int status, n, ns;
-            trace_ray<MODEL, H1, MULTI, FULLX>(P, alpha, beta, sI, sTau, sstride, I0, tau0, X, K, status, n, ns);
+            trace_ray<MODEL, H1, MULTI, FULLX, INTEG>(P, alpha, beta, sI, sTau, sstride, I0, tau0, X, K, status, n, ns);
             steps += (unsigned)n; sampled += (unsigned)ns; rays += 1;
             const size_t npix = O.alpha ? (size_t)O.nrays : (size_t)P.nx * P.ny;
             if (O.image) {
@@ -209,10 +248,10 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
     }
 }
 
-template <int MODEL, bool H1, bool MULTI, bool FULLX>
+template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG>
 static cudaError_t launch_one(const KP& P, const RenderOut& O, int grid, cudaStream_t stream) {
     size_t smem = MULTI ? (size_t)2 * P.n_freq * RAPTOR_BLOCK * sizeof(double) : 0;
-    auto kern = k_render<MODEL, H1, MULTI, FULLX>;
+    auto kern = k_render<MODEL, H1, MULTI, FULLX, INTEG>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -221,28 +260,29 @@ static cudaError_t launch_one(const KP& P, const RenderOut& O, int grid, cudaStr
     return cudaGetLastError();
 }
 
-template <int MODEL, bool FULLX>
+template <int MODEL, bool FULLX, int INTEG>
 static cudaError_t launch_hm(const KP& P, const RenderOut& O, bool h1, bool multi, int grid, cudaStream_t s) {
-    if (h1) return multi ? launch_one<MODEL, true, true, FULLX>(P, O, grid, s) : launch_one<MODEL, true, false, FULLX>(P, O, grid, s);
-    return multi ? launch_one<MODEL, false, true, FULLX>(P, O, grid, s) : launch_one<MODEL, false, false, FULLX>(P, O, grid, s);
+    if (h1) return multi ? launch_one<MODEL, true, true, FULLX, INTEG>(P, O, grid, s) : launch_one<MODEL, true, false, FULLX, INTEG>(P, O, grid, s);
+    return multi ? launch_one<MODEL, false, true, FULLX, INTEG>(P, O, grid, s) : launch_one<MODEL, false, false, FULLX, INTEG>(P, O, grid, s);
 }
 
-template <int MODEL>
+template <int MODEL, int INTEG>
 cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, cudaStream_t s) {
-    // the 3-D / slow-light sampler reads X^t, X^phi: always FULLX; the other models need them for the XK output only
-    if (MODEL == M_GRID3DT || fullx) return launch_hm<MODEL, true>(P, O, h1, multi, grid, s);
-    return launch_hm<MODEL, MODEL == M_GRID3DT>(P, O, h1, multi, grid, s);
+    // the 3-D / slow-light sampler reads X^t, X^phi: always FULLX; the other models need them for the XK output only.
+    // The second-order integrators (8(f) f1) are built in the FULLX form only.
+    if (MODEL == M_GRID3DT || fullx || INTEG != I_RK4) return launch_hm<MODEL, true, INTEG>(P, O, h1, multi, grid, s);
+    return launch_hm<MODEL, MODEL == M_GRID3DT || INTEG != I_RK4, INTEG>(P, O, h1, multi, grid, s);
 }
 
-#ifdef RAPTOR_MODEL
-template cudaError_t launch_model<RAPTOR_MODEL>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+// one translation unit per (plasma model, integrator): -DRAPTOR_MODEL=m -DRAPTOR_INTEG=i (build.py, in parallel);
+// without the macros, everything in this one
+#define RAPTOR_INST(M, I) template cudaError_t launch_model<M, I>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+#if defined(RAPTOR_MODEL) && defined(RAPTOR_INTEG)
+RAPTOR_INST(RAPTOR_MODEL, RAPTOR_INTEG)
 #else
-template cudaError_t launch_model<M_VACUUM>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
-template cudaError_t launch_model<M_SPHERE>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
-template cudaError_t launch_model<M_TORUS>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
-template cudaError_t launch_model<M_GRID2D>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
-template cudaError_t launch_model<M_GRID3DT>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
-template cudaError_t launch_model<M_SLAB>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+#define RAPTOR_INST_ALL(M) RAPTOR_INST(M, I_RK4) RAPTOR_INST(M, I_VERLET) RAPTOR_INST(M, I_VERLET_C) RAPTOR_INST(M, I_RK2)
+RAPTOR_INST_ALL(M_VACUUM) RAPTOR_INST_ALL(M_SPHERE) RAPTOR_INST_ALL(M_TORUS)
+RAPTOR_INST_ALL(M_GRID2D) RAPTOR_INST_ALL(M_GRID3DT) RAPTOR_INST_ALL(M_SLAB)
 #endif
 
 }  // namespace raptor

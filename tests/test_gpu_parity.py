@@ -264,3 +264,43 @@ def test_grid_upload_replaces_the_snapshot(rb):
         R.upload_grid(s.grid)
         f2 = R.spectrum().cpu().numpy()
     assert f1[0] > 1.05 * f0[0] and np.array_equal(f0, f2)        # (the source is optically thick at 230 GHz)
+
+
+# ------------------------------------------------- 8(f) f1: second-order integrators (Eq. 17-20, "RK2")
+@pytest.mark.parametrize("integ", [1, 2, 3])
+@pytest.mark.parametrize("cfg", ["C1", "C2", "C4"])
+def test_second_order_integrators_full_parity(rb, orc, integ, cfg):
+    if cfg == "C1":
+        s = replace(scenes.config_C1(64), nx=44, ny=26)
+    elif cfg == "C2":
+        s = scenes.config_C2(nx=40)
+    else:
+        s = scenes.config_C4(nx=24, n1=48, n2=32, n3=16, nt=8)
+    check_full(rb, orc, replace(s, integrator=integ))
+
+
+@pytest.mark.parametrize("integ", [1, 2, 3])
+def test_second_order_integrators_policy_B_spectrum(rb, orc, integ):
+    # the paper's performance configuration (Table B.1): step rule Eq. 21-24 with eps = 0.03
+    s = replace(scenes.config_C3(nx=20, n_freq=4), integrator=integ, step_policy=1, eps=0.03, max_steps=50000)
+    g = gpu_render(rb, s)
+    ref = orc.Oracle(s).render()
+    keep = ~ring_mask(s, 0.15)
+    assert (g["status"][keep] == ref["status"][keep]).all()
+    assert (rel_err(g["image"], ref["image"])[:, keep] <= 1e-7).mean() >= 0.99
+
+
+@pytest.mark.parametrize("integ", [1, 2, 3])
+def test_second_order_integrators_single_rays(rb, orc, integ):
+    s = replace(scenes.config_C2(nx=8), integrator=integ)
+    rng = np.random.default_rng(17)
+    al, be = rng.uniform(-18, 18, 24), rng.uniform(-18, 18, 24)
+    with rb.Raptor(s) as R:
+        g = R.trace(al, be)
+    o = orc.Oracle(s)
+    for i in range(al.size):
+        r = o.trace(al[i], be[i])
+        assert g["status"][i] == r["status"] and g["nsteps"][i] == r["nsteps"], (i, al[i], be[i])
+        assert np.all(np.abs(g["XK"][i, :4] - r["X"]) <= 1e-8 * np.maximum(np.abs(r["X"]), 1.0))
+        assert np.all(np.abs(g["XK"][i, 4:] - r["K"]) <= 1e-8 * np.abs(r["K"]).max())
+        assert abs(g["I"][0, i] - r["I"][0]) <= 1e-8 * abs(r["I"][0]) + 1e-300
