@@ -71,7 +71,7 @@ typedef struct {
     /* plasma */
     double model[16];          /* SPHERE: n0, n_exp, T0[K], T_exp, beta.  TORUS: n_max, r_peak, r_halfwidth,
                                   scale height H, T0, T_exp, beta.  SLAB: n_e, Theta_e, B[G], half thickness, sin(pitch) */
-    double tp_over_te;         /* T_p/T_e (Table 2) */
+    double tp_over_te;         /* T_p/T_e (Table 2), te_model = 0 */
     double gamma_ad;           /* adiabatic index of the grid fluid */
     /* grid (GRID2D, GRID3DT): cell-centred, x1_i = x1_min + (i+1/2)(x1_max-x1_min)/n1, x2_j = (j+1/2)/n2,
      * phi_k = (k+1/2) 2pi/n3, t_m = t0 + m dt_snap [A16] */
@@ -85,12 +85,12 @@ typedef struct {
     int32_t max_steps;         /* per ray */
     int32_t n_freq;            /* 1 .. RAPTOR_MAX_FREQ */
     int32_t plasma_model;
-    int32_t k2_mode;           /* 0: K_2(1/Theta) = 2 Theta^2 */
+    int32_t k2_mode;           /* 0: K_2(1/Theta) = 2 Theta^2; 1: K_2 evaluated (Eq. 41-42 as written) */
     int32_t n1, n2, n3, nt;
     int32_t grid_dtype;        /* 0 = float64, 1 = float32 */
     int32_t slow_light;        /* 1: interpolate between snapshots at the ray's coordinate time */
     int32_t snapshot;          /* fast light: snapshot index used */
-    int32_t reserved_;
+    int32_t te_model;          /* 0: constant tp_over_te; 1: Eq. 47, model[0] = R_low, model[1] = R_high (grids) */
 } raptor_params;
 
 /* Validates and copies *p, uploads frequencies and grid.  *out is NULL on failure (then

@@ -63,7 +63,7 @@ typedef struct {
     const double *freq_hz;
     const void *grid;
     int32_t nx, ny, integrator, step_policy, max_steps, n_freq, plasma_model, k2_mode;
-    int32_t n1, n2, n3, nt, grid_dtype, slow_light, snapshot, pad_;
+    int32_t n1, n2, n3, nt, grid_dtype, slow_light, snapshot, te_model;
 } orc_params;
 
 /* ======================================================================================= */
@@ -563,7 +563,18 @@ int orc_plasma(const orc_params *P, const double X[4], double *ne, double *theta
     *ne = rho * rho0 / (ORC_MP + ORC_ME);                                      /* Eq. 46 */
     double bsq = dot4(g, p, p);
     *Bg = sqrt(bsq > 0.0 ? bsq : 0.0) * B0;
-    *thetae = (ORC_MP / ORC_ME) * (P->gamma_ad - 1.0) * (uu / rho) / (1.0 + P->tp_over_te);
+    /* T_p/T_e: constant (Table 2) or, te_model = 1, Eq. 47:
+     * R = R_low/(1+beta_p^2) + R_high beta_p^2/(1+beta_p^2), beta_p = P_gas/P_mag, P_gas = (gamma-1) u,
+     * P_mag = b^2/2 (code units); model[0] = R_low, model[1] = R_high.  b^2 = 0 is the limit beta_p -> inf. */
+    double R = P->tp_over_te;
+    if (P->te_model == 1) {
+        if (bsq > 0.0) {
+            double beta_p = (P->gamma_ad - 1.0) * uu / (0.5 * bsq);
+            double b2 = beta_p * beta_p;
+            R = M[0] * (1.0 / (1.0 + b2)) + M[1] * (b2 / (1.0 + b2));
+        } else R = M[1];
+    }
+    *thetae = (ORC_MP / ORC_ME) * (P->gamma_ad - 1.0) * (uu / rho) / (1.0 + R);
     return 1;
 }
 
@@ -599,6 +610,7 @@ double orc_emissivity(double nu, double ne, double thetae, double Bg, double sin
     if (!(nu_s > 0.0) || !(ne > 0.0)) return 0.0;                              /* [A13] */
     double Xx = nu / nu_s;                                                     /* Eq. 43 */
     double K2 = (k2_mode == 1) ? orc_bessel_k2(1.0 / thetae) : 2.0 * thetae * thetae;
+    if (!(K2 > 0.0)) return 0.0;                                               /* K_2 underflow (Theta_e < ~1/745) [A13] */
     double term = sqrt(Xx) + pow(2.0, 11.0 / 12.0) * pow(Xx, 1.0 / 6.0);
     return ne * (sqrt(2.0) * ORC_PI * ORC_E * ORC_E * nu_s / (3.0 * ORC_C * K2)) * term * term * exp(-cbrt(Xx));
 }

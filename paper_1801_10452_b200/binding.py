@@ -42,7 +42,7 @@ class RaptorParams(C.Structure):
         ("nx", C.c_int32), ("ny", C.c_int32), ("integrator", C.c_int32), ("step_policy", C.c_int32),
         ("max_steps", C.c_int32), ("n_freq", C.c_int32), ("plasma_model", C.c_int32), ("k2_mode", C.c_int32),
         ("n1", C.c_int32), ("n2", C.c_int32), ("n3", C.c_int32), ("nt", C.c_int32),
-        ("grid_dtype", C.c_int32), ("slow_light", C.c_int32), ("snapshot", C.c_int32), ("reserved_", C.c_int32),
+        ("grid_dtype", C.c_int32), ("slow_light", C.c_int32), ("snapshot", C.c_int32), ("te_model", C.c_int32),
     ]
 
 
@@ -100,7 +100,7 @@ def params_from_scene(scene):
                  "r_stop_out_factor", "tau_cutoff", "tp_over_te", "gamma_ad", "x1_min", "x1_max", "t0", "dt_snap"):
         setattr(p, name, float(getattr(scene, name)))
     for name in ("nx", "ny", "integrator", "step_policy", "max_steps", "plasma_model", "k2_mode",
-                 "n1", "n2", "n3", "nt", "grid_dtype", "slow_light", "snapshot"):
+                 "n1", "n2", "n3", "nt", "grid_dtype", "slow_light", "snapshot", "te_model"):
         setattr(p, name, int(getattr(scene, name)))
     m = list(scene.model) + [0.0] * 16
     p.model = (C.c_double * 16)(*m[:16])

@@ -99,7 +99,9 @@ static int validate(const raptor_params* p) {
     if (!(p->r_stop_in_factor > 0.0) || !(p->r_stop_out_factor >= 1.0)) return fail(nullptr, RAPTOR_EINVAL, "bad r_stop factors");
     if (std::isnan(p->tau_cutoff)) return fail(nullptr, RAPTOR_EINVAL, "tau_cutoff is NaN");
     if (p->plasma_model < 0 || p->plasma_model > 5) return fail(nullptr, RAPTOR_EINVAL, "unknown plasma_model %d", p->plasma_model);
-    if (p->k2_mode != 0) return fail(nullptr, RAPTOR_EUNSUPPORTED, "k2_mode %d: only 0 (K2 = 2 Theta^2, PAPER.md:303) is built", p->k2_mode);
+    if (p->k2_mode != 0 && p->k2_mode != 1) return fail(nullptr, RAPTOR_EINVAL, "k2_mode %d: 0 (K2 = 2 Theta^2, PAPER.md:303) or 1 (exact K2)", p->k2_mode);
+    if (p->te_model != 0 && p->te_model != 1) return fail(nullptr, RAPTOR_EINVAL, "te_model %d: 0 (constant T_p/T_e) or 1 (Eq. 47)", p->te_model);
+    if (p->te_model == 1 && !(p->model[0] >= 0.0 && p->model[1] >= 0.0)) return fail(nullptr, RAPTOR_EINVAL, "te_model 1 needs model[0] = R_low >= 0, model[1] = R_high >= 0");
     if (!(p->M_bh_g > 0.0) || !(p->D_src_cm > 0.0)) return fail(nullptr, RAPTOR_EINVAL, "M_bh_g and D_src_cm must be > 0");
     if (p->plasma_model == RAPTOR_GRID2D || p->plasma_model == RAPTOR_GRID3DT) {
         if (p->n1 < 2 || p->n2 < 2 || p->n3 < 1 || p->nt < 1) return fail(nullptr, RAPTOR_EINVAL, "grid dims: n1, n2 >= 2, n3, nt >= 1");
@@ -142,6 +144,7 @@ static void build_kp(raptor_ctx* c) {
     k.ne_scale = rho0 / (kMP + kME);                                     // Eq. 46
     k.B0 = kC * std::sqrt(4.0 * kPI * rho0);
     k.thetae_scale = (kMP / kME) * (p.gamma_ad - 1.0) / (1.0 + p.tp_over_te);
+    k.thetae_num = (kMP / kME) * (p.gamma_ad - 1.0); k.gm1 = p.gamma_ad - 1.0; k.te_model = p.te_model;
     for (int i = 0; i < 16; ++i) k.model[i] = p.model[i];
     if (p.n1 > 0) {
         const double d1 = (p.x1_max - p.x1_min) / p.n1;

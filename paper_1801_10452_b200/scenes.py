@@ -75,6 +75,7 @@ class Scene:
     model: tuple = (0.0,) * 16
     k2_mode: int = 0
     tp_over_te: float = 3.0
+    te_model: int = 0           # 0: constant T_p/T_e; 1: Eq. 47 with model[0] = R_low, model[1] = R_high (grids)
     gamma_ad: float = 4.0 / 3.0
     # grid (models GRID2D, GRID3DT): AoS [t][i1][i2][i3][8] = rho,u,u~1,u~2,u~3,B1,B2,B3
     n1: int = 0

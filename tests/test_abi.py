@@ -42,7 +42,7 @@ def test_struct_layout_matches_the_header(lib):
 @pytest.mark.parametrize("field,value,needle", [
     ("a", 1.0, "spin"), ("a", float("nan"), "spin"), ("incl_deg", 0.0, "inclination"), ("incl_deg", 180.0, "inclination"),
     ("nx", 0, "nx"), ("r_cam", 1.5, "r_cam"), ("mks_h", 0.0, "mks_h"), ("max_steps", 0, "max_steps"),
-    ("integrator", 4, "integrator"), ("k2_mode", 1, "k2_mode"), ("plasma_model", 9, "plasma_model"),
+    ("integrator", 4, "integrator"), ("k2_mode", 2, "k2_mode"), ("plasma_model", 9, "plasma_model"),
     ("step_min", 0.0, "policy A"), ("fov_M", -1.0, "fov_M"), ("tau_cutoff", float("nan"), "tau_cutoff"),
 ])
 def test_validation_rejects_bad_parameters(lib, field, value, needle):

@@ -304,3 +304,38 @@ def test_second_order_integrators_single_rays(rb, orc, integ):
         assert np.all(np.abs(g["XK"][i, :4] - r["X"]) <= 1e-8 * np.maximum(np.abs(r["X"]), 1.0))
         assert np.all(np.abs(g["XK"][i, 4:] - r["K"]) <= 1e-8 * np.abs(r["K"]).max())
         assert abs(g["I"][0, i] - r["I"][0]) <= 1e-8 * abs(r["I"][0]) + 1e-300
+
+
+# ------------------------------------------------- 8(f) f2: exact K_2, Eq. 47 electron temperatures
+def test_exact_bessel_k2_parity(rb, orc):
+    # series branch (x = 1/Theta_e <= 2 everywhere on the synthetic grid)
+    check_full(rb, orc, replace(scenes.config_C2(nx=40), k2_mode=1))
+    check_full(rb, orc, replace(scenes.config_C3(nx=16, n_freq=8), k2_mode=1))
+
+
+@pytest.mark.parametrize("theta_e", [3.0, 0.45, 0.2, 0.05, 0.011, 1e-3])
+def test_exact_bessel_k2_cold_plasma_slab(rb, orc, theta_e):
+    # x = 1/Theta_e from 0.33 (series) over 2.2 ... 91 (trapezoid branch) to 1000 (K_2 underflows: no emission)
+    s = replace(scenes.slab_scene(1e6, theta_e, 30.0, 8.0, step_c=0.0, step_min=0.25, step_max=0.25, eps_polar=1e30,
+                                  r_cam=60.0, incl_deg=30.0), k2_mode=1, freq_hz=(1e8, 1e9, 230e9))
+    with rb.Raptor(s) as R:
+        g = R.trace([4.0, -2.0], [3.0, 1.0])
+    o = orc.Oracle(s)
+    for i, (al, be) in enumerate([(4.0, 3.0), (-2.0, 1.0)]):
+        r = o.trace(al, be)
+        assert g["nsteps"][i] == r["nsteps"]
+        assert np.isfinite(g["I"][:, i]).all()
+        assert np.all(np.abs(g["I"][:, i] - r["I"]) <= 1e-10 * np.abs(r["I"]) + 1e-300), (g["I"][:, i], r["I"])
+        assert np.all(np.abs(g["tau"][:, i] - r["tau"]) <= 1e-10 * np.abs(r["tau"]) + 1e-300)
+    if theta_e == 1e-3:
+        assert (g["I"] == 0).all()
+
+
+@pytest.mark.parametrize("r_low,r_high", [(1.0, 25.0), (1.0, 1.0), (3.0, 80.0)])
+def test_electron_temperature_eq47_parity(rb, orc, r_low, r_high):
+    # the jet / disk models of PAPER.md:399-401 use (1, 25) and (1, 1)
+    model = (r_low, r_high) + (0.0,) * 14
+    g, ref, _ = check_full(rb, orc, replace(scenes.config_C2(nx=40), te_model=1, model=model))
+    check_full(rb, orc, replace(scenes.config_C4(nx=24, n1=48, n2=32, n3=16, nt=8), te_model=1, model=model))
+    base = gpu_render(rb, scenes.config_C2(nx=40))
+    assert abs(g["flux"][0] / base["flux"][0] - 1.0) > 1e-3        # the option does something

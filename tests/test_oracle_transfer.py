@@ -278,6 +278,43 @@ def test_grid_unit_scaling_eq46_and_electron_temperature():
     assert np.allclose(pl["p"][1:], (Bv[1:] + bt * pl["u"][1:]) / pl["u"][0], rtol=1e-11)
 
 
+def test_electron_temperature_ratio_eq47_limits_and_reduction():
+    # Eq. 47: T_p/T_e = R_low/(1+beta_p^2) + R_high beta_p^2/(1+beta_p^2), beta_p = P_gas/P_mag,
+    # P_mag = b^2/2.  Pinned by what the paper states about it: beta_p << 1 -> R_low, beta_p >> 1 -> R_high
+    # (PAPER.md:377), R_low = R_high = R is the constant-ratio model (the disk model of PAPER.md:399 has both = 1),
+    # and beta_p = 1 gives the mean of the two.
+    base = scenes.config_C2(nx=8, n1=32, n2=32)
+    d1 = (base.x1_max - base.x1_min) / base.n1
+    X = [0.0, base.x1_min + 20.5 * d1, 15.5 / base.n2, 0.3]
+    const = orc.Oracle(base).plasma(X)
+
+    def theta_e(grid, r_low, r_high):
+        s = replace(base, te_model=1, model=(r_low, r_high) + (0.0,) * 14, grid=grid)
+        return orc.Oracle(s).plasma(X)["theta_e"]
+
+    # R_low = R_high = tp_over_te: identical to the constant-ratio path, which test_grid_unit_scaling pins
+    assert theta_e(base.grid, 3.0, 3.0) == pytest.approx(const["theta_e"], rel=1e-14)
+    scale = (MP_ / ME_) * (base.gamma_ad - 1)
+    u_over_rho = base.grid[20, 15, 0, 1] / base.grid[20, 15, 0, 0]
+    weak, strong = base.grid.copy(), base.grid.copy()
+    weak[..., 5:] *= 1e-6          # b^2 -> 1e-12 b^2: beta_p >> 1
+    strong[..., 5:] *= 1e3         # beta_p << 1
+    assert theta_e(weak, 1.0, 25.0) == pytest.approx(scale * u_over_rho / (1 + 25.0), rel=1e-9)
+    assert theta_e(strong, 1.0, 25.0) == pytest.approx(scale * u_over_rho / (1 + 1.0), rel=1e-6)
+    # beta_p = 1 exactly: rescale the field so that b^2/2 = (gamma - 1) u at this cell (b^2 is quadratic in B^i)
+    o = orc.Oracle(base)
+    g = o.metric(X)
+    b2 = const["p"] @ g @ const["p"]
+    lam = math.sqrt((base.gamma_ad - 1) * base.grid[20, 15, 0, 1] / (0.5 * b2))
+    unit = base.grid.copy()
+    unit[..., 5:] *= lam
+    assert theta_e(unit, 1.0, 25.0) == pytest.approx(scale * u_over_rho / (1 + 13.0), rel=1e-10)
+    # zero field: the beta_p -> infinity limit
+    zero = base.grid.copy()
+    zero[..., 5:] = 0.0
+    assert theta_e(zero, 1.0, 25.0) == pytest.approx(scale * u_over_rho / 26.0, rel=1e-13)
+
+
 # ------------------------------------------------------------------------------------ P12
 def _linear_grid_scene(n1=12, n2=10, n3=8, nt=5, slow=True):
     """A grid whose 8 fields are multilinear in (x1, x2, t) and a trig polynomial in phi."""
