@@ -177,8 +177,18 @@ extern "C" int raptor_create(const raptor_params* p, raptor_ctx** out) {
     CKC(cudaGetDevice(&c->device));
     CKC(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
     CKC(cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking));
-    CKC(cudaMalloc(&c->d_freq, sizeof(double) * p->n_freq));
-    CKC(cudaMemcpy(c->d_freq, p->freq_hz, sizeof(double) * p->n_freq, cudaMemcpyHostToDevice));
+    {
+        // per-frequency constants of the transfer update: nu_k, nu_k^(1/6) (Eq. 43), c^2 / (2 h nu_k^3) (Eq. 45)
+        double tab[3 * RAPTOR_MAX_FREQ];
+        for (int k = 0; k < p->n_freq; ++k) {
+            const double nu = p->freq_hz[k];
+            tab[k] = nu;
+            tab[p->n_freq + k] = std::cbrt(std::sqrt(nu));
+            tab[2 * p->n_freq + k] = (kC * kC) / (2.0 * kHPL * nu * nu * nu);
+        }
+        CKC(cudaMalloc(&c->d_freq, sizeof(double) * 3 * p->n_freq));
+        CKC(cudaMemcpy(c->d_freq, tab, sizeof(double) * 3 * p->n_freq, cudaMemcpyHostToDevice));
+    }
     CKC(cudaMalloc(&c->d_queue, sizeof(unsigned int)));
     CKC(cudaMalloc(&c->d_counters, 3 * sizeof(unsigned long long)));
     CKC(cudaMemset(c->d_counters, 0, 3 * sizeof(unsigned long long)));

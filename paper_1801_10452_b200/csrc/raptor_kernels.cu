@@ -8,21 +8,36 @@
 
 namespace raptor {
 
+// Launch shape of the persistent ray kernel.  Single frequency: RAPTOR_MIN_BLOCKS CTAs of RAPTOR_BLOCK threads per
+// SM (16 warps, the register limit at 128 registers).  Several frequencies: I/tau take 16 n_freq bytes of shared
+// memory per thread, so the (CTAs per SM, warps per CTA) pair with the most resident warps that fits 228 KB per SM
+// (1 KB reserved per CTA) and 227 KB per CTA is used -- e.g. 2 x 7 warps at 32 frequencies: 148 x 14 = 2072 warp
+// slots, so the 2048 tiles of a 256^2 image (C3) run as a single wave.
+static void launch_shape(int n_freq, int& ctas_per_sm, int& warps_per_cta) {
+    ctas_per_sm = RAPTOR_MIN_BLOCKS; warps_per_cta = RAPTOR_BLOCK / 32;
+    if (n_freq <= 1) return;
+    const long long per_warp = 32ll * 16 * n_freq;
+    int best = 0;
+    for (int c = 1; c <= RAPTOR_MIN_BLOCKS; ++c) {
+        long long w = ((228ll * 1024) / c - 1024) / per_warp;
+        if (w * per_warp > 227ll * 1024) w = (227ll * 1024) / per_warp;
+        if (w > RAPTOR_BLOCK_MULTI / 32) w = RAPTOR_BLOCK_MULTI / 32;
+        if (c * w > 16) w = 16 / c;
+        if (w >= 1 && c * (int)w >= best) { best = c * (int)w; ctas_per_sm = c; warps_per_cta = (int)w; }
+    }
+    if (best == 0) { ctas_per_sm = 1; warps_per_cta = 1; }
+}
+
 cudaError_t launch_render(const KP& P, int model, const RenderOut& O, int sm_count, cudaStream_t stream) {
     const bool h1 = (P.omh == 0.0), multi = P.n_freq > 1;
-    // persistent grid: RAPTOR_MIN_BLOCKS CTAs per SM (fewer when shared memory for I/tau limits residency)
-    int per_sm = RAPTOR_MIN_BLOCKS;
-    if (multi) {
-        size_t smem = (size_t)2 * P.n_freq * RAPTOR_BLOCK * sizeof(double);
-        int fit = (int)((220u * 1024u) / (smem + 1024));
-        if (fit < 1) fit = 1;
-        if (fit < per_sm) per_sm = fit;
-    }
-    long long want = ((long long)O.ntiles * 32 + RAPTOR_BLOCK - 1) / RAPTOR_BLOCK;
+    int per_sm, warps;
+    launch_shape(P.n_freq, per_sm, warps);
+    const int block = warps * 32;
+    long long want = ((long long)O.ntiles + warps - 1) / warps;
     int grid = sm_count * per_sm;
     if (want < grid) grid = (int)(want > 0 ? want : 1);
     const bool fullx = O.XK != nullptr;
-#define RAPTOR_CASE_I(M, I) case I: return launch_model<M, I>(P, O, h1, multi, fullx, grid, stream);
+#define RAPTOR_CASE_I(M, I) case I: return launch_model<M, I>(P, O, h1, multi, fullx, grid, block, stream);
 #define RAPTOR_CASE_M(M)                                                                          \
     case M:                                                                                       \
         switch (P.integrator) {                                                                   \

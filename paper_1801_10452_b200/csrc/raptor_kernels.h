@@ -9,6 +9,10 @@
 #ifndef RAPTOR_BLOCK
 #define RAPTOR_BLOCK 128
 #endif
+// with several frequencies a CTA may have up to RAPTOR_BLOCK_MULTI threads (see launch_shape in raptor_kernels.cu)
+#ifndef RAPTOR_BLOCK_MULTI
+#define RAPTOR_BLOCK_MULTI 256
+#endif
 #ifndef RAPTOR_MIN_BLOCKS
 #define RAPTOR_MIN_BLOCKS 4
 #endif
@@ -33,7 +37,7 @@ struct RenderOut {
 
 // raptor_render.cu: one explicit instantiation per (plasma model, integrator), one translation unit each
 template <int MODEL, int INTEG>
-cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, cudaStream_t s);
+cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, int block, cudaStream_t s);
 cudaError_t launch_render(const KP& P, int model, const RenderOut& O, int sm_count, cudaStream_t stream);
 int flux_chunks(size_t npix);
 cudaError_t launch_flux(const double* d_image, size_t npix, int n_freq, double scale, double* d_partial,

@@ -161,13 +161,25 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
                 EmisConst E;
                 emis_prepare(P, pl, h, E);
                 if (MULTI) {
-                    for (int k = 0; k < P.n_freq; ++k) {
-                        double Ik = sI[k * sstride], tk = sTau[k * sstride];
-                        transfer_one(pl, E, __ldg(P.freq + k), Ik, tk);
-                        sI[k * sstride] = Ik; sTau[k * sstride] = tk;
+                    // two frequencies per iteration: their (branch-free) updates are independent chains
+                    const int nf = P.n_freq;
+                    const double* __restrict__ fq = P.freq;
+                    int k = 0;
+                    for (; k + 1 < nf; k += 2) {
+                        double Ia = sI[k * sstride], ta = sTau[k * sstride];
+                        double Ib = sI[(k + 1) * sstride], tb = sTau[(k + 1) * sstride];
+                        transfer_one(pl, E, __ldg(fq + k), __ldg(fq + nf + k), __ldg(fq + 2 * nf + k), Ia, ta);
+                        transfer_one(pl, E, __ldg(fq + k + 1), __ldg(fq + nf + k + 1), __ldg(fq + 2 * nf + k + 1), Ib, tb);
+                        sI[k * sstride] = Ia; sTau[k * sstride] = ta;
+                        sI[(k + 1) * sstride] = Ib; sTau[(k + 1) * sstride] = tb;
+                    }
+                    if (k < nf) {
+                        double Ia = sI[k * sstride], ta = sTau[k * sstride];
+                        transfer_one(pl, E, __ldg(fq + k), __ldg(fq + nf + k), __ldg(fq + 2 * nf + k), Ia, ta);
+                        sI[k * sstride] = Ia; sTau[k * sstride] = ta;
                     }
                 } else {
-                    transfer_one(pl, E, __ldg(P.freq), I, tau);
+                    transfer_one(pl, E, __ldg(P.freq), __ldg(P.freq + 1), __ldg(P.freq + 2), I, tau);
                 }
             }
         }
@@ -180,7 +192,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
 // Persistent-warp driver: tiles of 8x4 pixels (render) or 32 consecutive rays (trace) from a global queue.
 // --------------------------------------------------------------------------------------------
 template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG>
-__global__ void __launch_bounds__(RAPTOR_BLOCK, RAPTOR_MIN_BLOCKS)
+__global__ void __launch_bounds__(MULTI ? RAPTOR_BLOCK_MULTI : RAPTOR_BLOCK, MULTI ? (RAPTOR_BLOCK * RAPTOR_MIN_BLOCKS) / RAPTOR_BLOCK_MULTI : RAPTOR_MIN_BLOCKS)
 k_render(const __grid_constant__ KP P, const RenderOut O) {
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31;
@@ -249,34 +261,34 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
 }
 
 template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG>
-static cudaError_t launch_one(const KP& P, const RenderOut& O, int grid, cudaStream_t stream) {
-    size_t smem = MULTI ? (size_t)2 * P.n_freq * RAPTOR_BLOCK * sizeof(double) : 0;
+static cudaError_t launch_one(const KP& P, const RenderOut& O, int grid, int block, cudaStream_t stream) {
+    size_t smem = MULTI ? (size_t)2 * P.n_freq * block * sizeof(double) : 0;
     auto kern = k_render<MODEL, H1, MULTI, FULLX, INTEG>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    kern<<<grid, RAPTOR_BLOCK, smem, stream>>>(P, O);
+    kern<<<grid, block, smem, stream>>>(P, O);
     return cudaGetLastError();
 }
 
 template <int MODEL, bool FULLX, int INTEG>
-static cudaError_t launch_hm(const KP& P, const RenderOut& O, bool h1, bool multi, int grid, cudaStream_t s) {
-    if (h1) return multi ? launch_one<MODEL, true, true, FULLX, INTEG>(P, O, grid, s) : launch_one<MODEL, true, false, FULLX, INTEG>(P, O, grid, s);
-    return multi ? launch_one<MODEL, false, true, FULLX, INTEG>(P, O, grid, s) : launch_one<MODEL, false, false, FULLX, INTEG>(P, O, grid, s);
+static cudaError_t launch_hm(const KP& P, const RenderOut& O, bool h1, bool multi, int grid, int block, cudaStream_t s) {
+    if (h1) return multi ? launch_one<MODEL, true, true, FULLX, INTEG>(P, O, grid, block, s) : launch_one<MODEL, true, false, FULLX, INTEG>(P, O, grid, block, s);
+    return multi ? launch_one<MODEL, false, true, FULLX, INTEG>(P, O, grid, block, s) : launch_one<MODEL, false, false, FULLX, INTEG>(P, O, grid, block, s);
 }
 
 template <int MODEL, int INTEG>
-cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, cudaStream_t s) {
+cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, int block, cudaStream_t s) {
     // the 3-D / slow-light sampler reads X^t, X^phi: always FULLX; the other models need them for the XK output only.
     // The second-order integrators (8(f) f1) are built in the FULLX form only.
-    if (MODEL == M_GRID3DT || fullx || INTEG != I_RK4) return launch_hm<MODEL, true, INTEG>(P, O, h1, multi, grid, s);
-    return launch_hm<MODEL, MODEL == M_GRID3DT || INTEG != I_RK4, INTEG>(P, O, h1, multi, grid, s);
+    if (MODEL == M_GRID3DT || fullx || INTEG != I_RK4) return launch_hm<MODEL, true, INTEG>(P, O, h1, multi, grid, block, s);
+    return launch_hm<MODEL, MODEL == M_GRID3DT || INTEG != I_RK4, INTEG>(P, O, h1, multi, grid, block, s);
 }
 
 // one translation unit per (plasma model, integrator): -DRAPTOR_MODEL=m -DRAPTOR_INTEG=i (build.py, in parallel);
 // without the macros, everything in this one
-#define RAPTOR_INST(M, I) template cudaError_t launch_model<M, I>(const KP&, const RenderOut&, bool, bool, bool, int, cudaStream_t);
+#define RAPTOR_INST(M, I) template cudaError_t launch_model<M, I>(const KP&, const RenderOut&, bool, bool, bool, int, int, cudaStream_t);
 #if defined(RAPTOR_MODEL) && defined(RAPTOR_INTEG)
 RAPTOR_INST(RAPTOR_MODEL, RAPTOR_INTEG)
 #else
