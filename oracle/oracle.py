@@ -75,6 +75,10 @@ def lib():
         _lib.orc_bessel_k2.restype = C.c_double
         _lib.orc_bessel_k2.argtypes = [C.c_double]
         _lib.orc_horizon.restype = C.c_double
+        _lib.orc_r_isco.restype = C.c_double
+        _lib.orc_r_isco.argtypes = [C.c_double]
+        _lib.orc_line_profile.argtypes = [C.POINTER(OrcParams), C.c_void_p, C.c_void_p, C.c_int, C.c_double,
+                                          C.c_double, C.c_void_p]
         _lib.orc_sizeof_params.restype = C.c_size_t
         _lib.orc_transfer_update.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)] + [C.c_double] * 5
         _lib.orc_mks_theta.argtypes = [C.c_double, C.c_double] + [C.POINTER(C.c_double)] * 3
@@ -231,6 +235,27 @@ class Oracle:
             out["path"] = path[:min(res.nsteps, max_path)]
         return out
 
+    def render_disk(self):
+        """Thin-disk workload: dict(image = sum of g^p/r^2 over counted crossings, redshift = g of the first one)."""
+        p = self.p
+        image = np.zeros((1, p.ny, p.nx))
+        red = np.zeros((1, p.ny, p.nx))
+        status = np.zeros((p.ny, p.nx), dtype=np.int32)
+        nsteps = np.zeros((p.ny, p.nx), dtype=np.int32)
+        steps, sampled = C.c_uint64(), C.c_uint64()
+        self.lib.orc_render_rows2(C.byref(p), image.ctypes.data_as(C.c_void_p), red.ctypes.data_as(C.c_void_p),
+                                  status.ctypes.data_as(C.c_void_p), nsteps.ctypes.data_as(C.c_void_p), 0, int(p.ny), 1,
+                                  C.byref(steps), C.byref(sampled))
+        return dict(image=image, redshift=red, status=status, nsteps=nsteps, steps=steps.value, sampled=sampled.value)
+
+    def line_profile(self, image_I, image_g, nbins, g_min, g_max):
+        a = np.ascontiguousarray(image_I, dtype=np.float64)
+        b = np.ascontiguousarray(image_g, dtype=np.float64)
+        hist = np.zeros(int(nbins))
+        self.lib.orc_line_profile(C.byref(self.p), a.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p), int(nbins),
+                                  float(g_min), float(g_max), hist.ctypes.data_as(C.c_void_p))
+        return hist
+
     def render(self, rows=None, row_stride: int = 1):
         """Full image (or rows [row0,row1) with a stride).  Returns dict(image, status, nsteps, steps, sampled)."""
         p = self.p
@@ -258,6 +283,10 @@ def planck(nu, theta_e):
 
 def emissivity(nu, n_e, theta_e, B, sin_th, k2_mode=0):
     return lib().orc_emissivity(float(nu), float(n_e), float(theta_e), float(B), float(sin_th), int(k2_mode))
+
+
+def r_isco(a):
+    return lib().orc_r_isco(float(a))
 
 
 def bessel_k2(x):

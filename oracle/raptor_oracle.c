@@ -48,7 +48,7 @@
 #define ORC_HPL    6.62607015e-27
 #define ORC_PI     3.14159265358979323846
 
-enum { ORC_VACUUM = 0, ORC_SPHERE = 1, ORC_TORUS = 2, ORC_GRID2D = 3, ORC_GRID3DT = 4, ORC_SLAB = 5 };
+enum { ORC_VACUUM = 0, ORC_SPHERE = 1, ORC_TORUS = 2, ORC_GRID2D = 3, ORC_GRID3DT = 4, ORC_SLAB = 5, ORC_DISK = 6 };
 enum { ORC_RUNNING = 0, ORC_CAPTURED = 1, ORC_ESCAPED = 2, ORC_MAXSTEPS = 3, ORC_THICK = 4, ORC_NONFINITE = 5 };
 
 typedef struct {
@@ -655,6 +655,55 @@ int orc_transfer(const orc_params *P, const double X[4], const double K[4], doub
 }
 
 /* ======================================================================================= */
+/* Thin-disk workload, Sect. 4.2.1 (Fig. 5-6) [A24]     */
+/* ======================================================================================= */
+/* Innermost stable circular orbit of the equatorial Kerr geodesics (Bardeen, Press & Teukolsky 1972, the
+ * reference the paper gives at PAPER.md:267); a > 0: prograde disk, a < 0: retrograde. */
+double orc_r_isco(double a)
+{
+    double z1 = 1.0 + cbrt(1.0 - a * a) * (cbrt(1.0 + a) + cbrt(1.0 - a));
+    double z2 = sqrt(3.0 * a * a + z1 * z1);
+    double sg = (a > 0.0) - (a < 0.0);
+    return 3.0 + z2 - sg * sqrt((3.0 - z1) * (3.0 + z1 + 2.0 * z2));
+}
+
+/* One step of a ray went from (Xp, Kp) to (X, K).  The equatorial plane is x2 = 1/2 (mod 1) in every MKS(h)
+ * chart (A.11: theta(1/2 + n) = pi/2 + n pi).  If the step crossed it, the crossing state is the linear
+ * interpolation of the MKS state in the step, the emitter is the circular equatorial geodesic
+ * u = u^t (1, 0, 0, Omega), Omega = 1/(r^{3/2} + a), and the redshift factor is g = nu_obs/nu_em = 1/(-k.u)
+ * (Eq. 31, E = 1).  model = [r_in (<= 0: ISCO), r_out, max_order, p]: a crossing of order
+ * n <= max_order with r_in <= r <= r_out adds g^p r^-2 (emission coefficient ~ 1/r^2, no absorption,
+ * PAPER.md:267; p = 3 is Eq. 32).  Returns 1 if the plane was crossed; *counted = 1 if it added. */
+int orc_disk_crossing(const orc_params *P, const double Xp[4], const double Kp[4], const double X[4],
+                      const double K[4], int order, double *dI, double *g_out, double *r_out_x, int *counted)
+{
+    double fa = floor(Xp[2] - 0.5), fb = floor(X[2] - 0.5);
+    *counted = 0;
+    if (fa == fb) return 0;
+    double plane = 0.5 + (fa > fb ? fa : fb);
+    double w = (plane - Xp[2]) / (X[2] - Xp[2]);
+    double Xc[4], Kc[4];
+    for (int i = 0; i < 4; ++i) { Xc[i] = Xp[i] + w * (X[i] - Xp[i]); Kc[i] = Kp[i] + w * (K[i] - Kp[i]); }
+    Xc[2] = plane;
+    double r = P->mks_r0 + exp(Xc[1]);
+    double r_in = P->model[0] > 0.0 ? P->model[0] : orc_r_isco(P->a);
+    *r_out_x = r;
+    if (order > (int)P->model[2] || !(r >= r_in) || !(r <= P->model[1])) return 1;
+    double g[4][4], u[4];
+    orc_metric_mks(P, Xc, g);
+    double Om = 1.0 / (pow(r, 1.5) + P->a);
+    double den = -g[0][0] - 2.0 * Om * g[0][3] - Om * Om * g[3][3];
+    if (!(den > 0.0)) return 1;
+    u[0] = 1.0 / sqrt(den); u[1] = 0.0; u[2] = 0.0; u[3] = u[0] * Om;
+    double nu_hat = -dot4(g, Kc, u);
+    double gg = 1.0 / nu_hat;
+    *dI = pow(gg, P->model[3]) / (r * r);
+    *g_out = gg;
+    *counted = 1;
+    return 1;
+}
+
+/* ======================================================================================= */
 /* Ray loop O4 and image driver                                                              */
 /* ======================================================================================= */
 typedef struct {
@@ -671,7 +720,7 @@ void orc_trace_ray(const orc_params *P, double alpha, double beta, double *I, do
     double X[4], K[4];
     const double rH = horizon_radius(P);
     const double r_in = P->r_stop_in_factor * rH, r_out = P->r_stop_out_factor * P->r_cam;
-    int n = 0, ns = 0, status = ORC_RUNNING;
+    int n = 0, ns = 0, ncross = 0, status = ORC_RUNNING;
     double nmax = 0.0;
     orc_camera_ab(P, alpha, beta, X, K);
     for (int k = 0; k < P->n_freq; ++k) { I[k] = 0.0; tau[k] = 0.0; }
@@ -686,6 +735,8 @@ void orc_trace_ray(const orc_params *P, double alpha, double beta, double *I, do
             if (tmin > P->tau_cutoff) { status = ORC_THICK; break; }
         }
         double h = orc_step_size(P, X, K);
+        double Xp[4], Kp[4];
+        memcpy(Xp, X, 32); memcpy(Kp, K, 32);
         orc_step(P, X, K, -h);                                                 /* backward [A2] */
         ++n;
         int fin = 1;
@@ -693,6 +744,14 @@ void orc_trace_ray(const orc_params *P, double alpha, double beta, double *I, do
         if (!fin) { status = ORC_NONFINITE; break; }
         if (path && n <= max_path) { memcpy(path + 8 * (n - 1), X, 32); memcpy(path + 8 * (n - 1) + 4, K, 32); }
         double rn = P->mks_r0 + exp(X[1]);
+        if (P->plasma_model == ORC_DISK) {
+            /* thin disk: I[0] = sum of g^p / r^2 over the counted crossings, tau[0] = g of the first counted one */
+            double dI, gg, rx; int counted;
+            if (orc_disk_crossing(P, Xp, Kp, X, K, ncross + 1, &dI, &gg, &rx, &counted)) {
+                ++ncross;
+                if (counted) { I[0] += dI; if (ns == 0) tau[0] = gg; ++ns; }
+            }
+        } else
         if (rn >= r_in && rn <= r_out) ns += orc_transfer(P, X, K, h, I, tau); /* [A8] end-point sample */
         if (monitor_null) { double nn = fabs(orc_null_norm(P, X, K)); if (nn > nmax) nmax = nn; }
     }
@@ -705,8 +764,18 @@ void orc_trace_ray(const orc_params *P, double alpha, double beta, double *I, do
 /* O8: image[k][iy][ix] = I_nu,obs [erg s^-1 cm^-2 Hz^-1 sr^-1] for rows row0 <= iy < row1 in
  * steps of row_stride (a stride > 1 is used only for bounded timing samples); status / nsteps
  * ([ny][nx]) may be NULL.  Parallel over image rows only.  *steps, *sampled: totals. */
+int orc_render_rows2(const orc_params *P, double *image, double *tau_image, int32_t *status, int32_t *nsteps,
+                     int row0, int row1, int row_stride, uint64_t *steps, uint64_t *sampled);
 int orc_render_rows(const orc_params *P, double *image, int32_t *status, int32_t *nsteps,
                     int row0, int row1, int row_stride, uint64_t *steps, uint64_t *sampled)
+{
+    return orc_render_rows2(P, image, NULL, status, nsteps, row0, row1, row_stride, steps, sampled);
+}
+
+/* as orc_render_rows; tau_image ([n_freq][ny][nx] or NULL) receives tau_k of every ray (thin disk: the
+ * redshift factor g of the first counted crossing, 0 if none) */
+int orc_render_rows2(const orc_params *P, double *image, double *tau_image, int32_t *status, int32_t *nsteps,
+                     int row0, int row1, int row_stride, uint64_t *steps, uint64_t *sampled)
 {
     uint64_t tot = 0, tots = 0;
     if (row_stride < 1) row_stride = 1;
@@ -719,6 +788,7 @@ int orc_render_rows(const orc_params *P, double *image, int32_t *status, int32_t
             orc_pixel_ab(P, ix, iy, &al, &be);
             orc_trace_ray(P, al, be, I, tau, &res, NULL, 0, 0);
             for (int k = 0; k < P->n_freq; ++k) image[((size_t)k * P->ny + iy) * P->nx + ix] = I[k];
+            if (tau_image) for (int k = 0; k < P->n_freq; ++k) tau_image[((size_t)k * P->ny + iy) * P->nx + ix] = tau[k];
             if (status) status[(size_t)iy * P->nx + ix] = res.status;
             if (nsteps) nsteps[(size_t)iy * P->nx + ix] = res.nsteps;
             tot += (uint64_t)res.nsteps; tots += (uint64_t)res.nsampled;
@@ -748,6 +818,24 @@ void orc_flux(const orc_params *P, const double *image, double *flux_jy)
             c = (t - s) - y; s = t;
         }
         flux_jy[k] = s * scale;
+    }
+}
+
+/* Line profile of the thin disk (Fig. 6): hist[b] = sum over pixels whose redshift factor g falls
+ * in bin b of [g_min, g_max) of I * (fov/nx)(fov/ny); pixels with g = 0 (no crossing) are skipped.  Row-major
+ * order, plain summation per bin. */
+void orc_line_profile(const orc_params *P, const double *image_I, const double *image_g, int nbins,
+                      double g_min, double g_max, double *hist)
+{
+    size_t npix = (size_t)P->nx * P->ny;
+    double area = (P->fov_M / P->nx) * (P->fov_M / P->ny);
+    for (int b = 0; b < nbins; ++b) hist[b] = 0.0;
+    for (size_t i = 0; i < npix; ++i) {
+        double g = image_g[i];
+        if (!(g > 0.0)) continue;
+        double fb = floor((g - g_min) / (g_max - g_min) * nbins);
+        if (fb < 0.0 || fb >= (double)nbins) continue;
+        hist[(int)fb] += image_I[i] * area;
     }
 }
 

@@ -30,7 +30,7 @@ M_P_G = 1.67262192e-24
 M_E_G = 9.1093837e-28
 
 # plasma_model codes (same numbering on both sides of the C ABI, include/raptor.h)
-VACUUM, SPHERE, TORUS, GRID2D, GRID3DT, SLAB = 0, 1, 2, 3, 4, 5
+VACUUM, SPHERE, TORUS, GRID2D, GRID3DT, SLAB, DISK = 0, 1, 2, 3, 4, 5, 6
 # grid_dtype codes
 F64, F32 = 0, 1
 
@@ -296,6 +296,17 @@ def slab_scene(n_e: float, theta_e: float, B_gauss: float, thickness_M: float,
                 nx=nx, ny=nx, plasma_model=SLAB, freq_hz=(nu_hz,),
                 model=(n_e, theta_e, B_gauss, 0.5 * thickness_M, sin_pitch) + (0.0,) * 11,
                 r_stop_in_factor=1.01, r_stop_out_factor=1.1)
+    base.update(kw)
+    return Scene(**base)
+
+
+def thin_disk(a: float = 0.0, incl_deg: float = 60.0, nx: int = 256, r_out: float = 15.0, max_order: int = 10,
+              p: float = 3.0, r_in: float = 0.0, **kw) -> Scene:
+    """Thin-disk workload of Sect. 4.2.1: equatorial Keplerian disk from the ISCO (r_in <= 0)
+    to 15 M, emission coefficient ~ 1/r^2, no absorption; lensed images up to ``max_order`` (Fig. 5: 10; the line
+    spectra of Fig. 6 use 1).  model = [r_in, r_out, max_order, p]"""
+    base = dict(name="thin_disk", a=a, mks_h=1.0, incl_deg=incl_deg, r_cam=1000.0, fov_M=40.0, nx=nx, ny=nx,
+                plasma_model=DISK, model=(r_in, r_out, float(max_order), p) + (0.0,) * 12)
     base.update(kw)
     return Scene(**base)
 
