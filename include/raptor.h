@@ -31,7 +31,8 @@ enum {
 };
 
 /* plasma_model */
-enum { RAPTOR_VACUUM = 0, RAPTOR_SPHERE = 1, RAPTOR_TORUS = 2, RAPTOR_GRID2D = 3, RAPTOR_GRID3DT = 4, RAPTOR_SLAB = 5 };
+enum { RAPTOR_VACUUM = 0, RAPTOR_SPHERE = 1, RAPTOR_TORUS = 2, RAPTOR_GRID2D = 3, RAPTOR_GRID3DT = 4, RAPTOR_SLAB = 5,
+       RAPTOR_DISK = 6 /* thin-disk workload of Sect. 4.2.1: raptor_render_disk */ };
 /* per-ray status word written by raptor_render */
 enum { RAPTOR_RUNNING = 0, RAPTOR_CAPTURED = 1, RAPTOR_ESCAPED = 2, RAPTOR_MAXSTEPS = 3, RAPTOR_THICK = 4, RAPTOR_NONFINITE = 5 };
 
@@ -70,7 +71,8 @@ typedef struct {
     double tau_cutoff;         /* stop when min_k tau_k exceeds it; +inf = off */
     /* plasma */
     double model[16];          /* SPHERE: n0, n_exp, T0[K], T_exp, beta.  TORUS: n_max, r_peak, r_halfwidth,
-                                  scale height H, T0, T_exp, beta.  SLAB: n_e, Theta_e, B[G], half thickness, sin(pitch) */
+                                  scale height H, T0, T_exp, beta.  SLAB: n_e, Theta_e, B[G], half thickness, sin(pitch).
+                                  DISK: r_in (<= 0: ISCO), r_out, max image order, p.  Grids with te_model = 1: R_low, R_high */
     double tp_over_te;         /* T_p/T_e (Table 2), te_model = 0 */
     double gamma_ad;           /* adiabatic index of the grid fluid */
     /* grid (GRID2D, GRID3DT): cell-centred, x1_i = x1_min + (i+1/2)(x1_max-x1_min)/n1, x2_j = (j+1/2)/n2,
@@ -106,6 +108,23 @@ int raptor_upload_grid(raptor_ctx *ctx, const void *grid_host, uint64_t grid_byt
  *   d_status device, [ny][nx] int32 status word, or NULL
  *   d_nsteps device, [ny][nx] int32 accepted RK4 steps of the ray, or NULL */
 int raptor_render(raptor_ctx *ctx, double *d_image, int32_t *d_status, int32_t *d_nsteps, void *cuda_stream);
+
+/* Thin-disk workload (Sect. 4.2.1; plasma_model = RAPTOR_DISK, n_freq = 1) [A24]: a steady,
+ * geometrically thin Keplerian disk in the equatorial plane between r_in (the ISCO) and r_out with emission
+ * coefficient ~ 1/r^2 and no absorption.  Every crossing of the equatorial plane of order <= max order inside
+ * [r_in, r_out] adds g^p / r^2, g = nu_obs/nu_em = 1/(-k.u) (Eq. 31-32); crossing state by linear
+ * interpolation within the step.
+ *   d_image    device, [ny][nx] float64: sum over the counted crossings (arbitrary units)
+ *   d_redshift device, [ny][nx] float64: g of the first counted crossing, 0 where there is none
+ *   d_status, d_nsteps as raptor_render (or NULL) */
+int raptor_render_disk(raptor_ctx *ctx, double *d_image, double *d_redshift, int32_t *d_status, int32_t *d_nsteps,
+                       void *cuda_stream);
+
+/* Line profile of the disk (Fig. 6): d_hist device [nbins], bin b of [g_min, g_max) receives
+ * sum I (fov/nx)(fov/ny) over the pixels whose redshift factor falls into it (g = 0 pixels are skipped).
+ * Fixed summation order (deterministic). */
+int raptor_line_profile(raptor_ctx *ctx, const double *d_image, const double *d_redshift, int32_t nbins, double g_min,
+                        double g_max, double *d_hist, void *cuda_stream);
 
 /* Multi-GPU sharding of one image: after this call raptor_render / raptor_spectrum /
  * raptor_render_host trace only the 8x4-pixel tiles rank, rank + world, rank + 2 world, ... (row-major tile

@@ -21,7 +21,8 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
 STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 5: "NONFINITE"}
 
 # every symbol include/raptor.h declares
-SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_spectrum", "raptor_flux",
+SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_render_disk",
+           "raptor_line_profile", "raptor_spectrum", "raptor_flux",
            "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_get_counters", "raptor_fp64_peak",
            "raptor_destroy", "raptor_last_error")
 
@@ -68,6 +69,8 @@ def lib():
         L.raptor_upload_grid.argtypes = [vp, vp, C.c_uint64, vp]
         L.raptor_set_shard.argtypes = [vp, i32, i32]
         L.raptor_render.argtypes = [vp, vp, vp, vp, vp]
+        L.raptor_render_disk.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.raptor_line_profile.argtypes = [vp, vp, vp, i32, C.c_double, C.c_double, vp, vp]
         L.raptor_spectrum.argtypes = [vp, vp, vp, vp]
         L.raptor_flux.argtypes = [vp, vp, vp, vp]
         L.raptor_render_host.argtypes = [vp, vp, vp, vp, vp]
@@ -130,6 +133,14 @@ def raptor_destroy(ctx):
 
 def raptor_render(ctx, d_image, d_status=None, d_nsteps=None, stream=None):
     _check(lib().raptor_render(ctx, d_image, d_status, d_nsteps, stream), ctx)
+
+
+def raptor_render_disk(ctx, d_image, d_redshift, d_status=None, d_nsteps=None, stream=None):
+    _check(lib().raptor_render_disk(ctx, d_image, d_redshift, d_status, d_nsteps, stream), ctx)
+
+
+def raptor_line_profile(ctx, d_image, d_redshift, nbins, g_min, g_max, d_hist, stream=None):
+    _check(lib().raptor_line_profile(ctx, d_image, d_redshift, int(nbins), float(g_min), float(g_max), d_hist, stream), ctx)
 
 
 def raptor_set_shard(ctx, rank, world):
@@ -213,6 +224,22 @@ class Raptor:
         raptor_render(self.ctx, image.data_ptr(), status.data_ptr() if want_status else None,
                       nsteps.data_ptr() if want_status else None, _stream_ptr())
         return (image, status, nsteps) if want_status else image
+
+    def render_disk(self):
+        """Thin-disk workload: (image [ny][nx], redshift [ny][nx], status, nsteps) as CUDA tensors."""
+        import torch
+        image = torch.empty((self.ny, self.nx), dtype=torch.float64, device="cuda")
+        red = torch.empty((self.ny, self.nx), dtype=torch.float64, device="cuda")
+        status = torch.empty((self.ny, self.nx), dtype=torch.int32, device="cuda")
+        nsteps = torch.empty((self.ny, self.nx), dtype=torch.int32, device="cuda")
+        raptor_render_disk(self.ctx, image.data_ptr(), red.data_ptr(), status.data_ptr(), nsteps.data_ptr(), _stream_ptr())
+        return image, red, status, nsteps
+
+    def line_profile(self, image, redshift, nbins, g_min, g_max):
+        import torch
+        hist = torch.empty((int(nbins),), dtype=torch.float64, device="cuda")
+        raptor_line_profile(self.ctx, image.data_ptr(), redshift.data_ptr(), nbins, g_min, g_max, hist.data_ptr(), _stream_ptr())
+        return hist
 
     def set_shard(self, rank, world):
         raptor_set_shard(self.ctx, rank, world)

@@ -1,7 +1,7 @@
 """Build of the C-ABI shared library ``libraptor_b200.so`` (in-tree, next to this file) with nvcc for sm_100a.
 
 The ray kernel (csrc/raptor_render.cu) is compiled once per (plasma model, integrator)
-(-DRAPTOR_MODEL=0..5 -DRAPTOR_INTEG=0..3) in parallel;
+(-DRAPTOR_MODEL=0..6 -DRAPTOR_INTEG=0..3) in parallel;
 objects go to ``build/`` (git-ignored) and are linked with the API and the satellite kernels.
 """
 from __future__ import annotations
@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libraptor_b200.so")
-N_MODELS = 6
+N_MODELS = 7
 N_INTEG = 4
 HEADERS = ["raptor_device.cuh", "raptor_kernels.h", os.path.join("..", "..", "include", "raptor.h")]
 SOURCES = ["raptor_render.cu", "raptor_kernels.cu", "raptor_api.cu"]

@@ -23,6 +23,8 @@ struct raptor_ctx {
     unsigned int* d_queue = nullptr;
     unsigned long long* d_counters = nullptr;
     double* d_partial = nullptr;      // flux partial sums [n_freq][chunks]
+    double* d_profile_partial = nullptr;   // line-profile partial sums [nbins][chunks]
+    int profile_bins = 0;
     double* d_scratch_image = nullptr;
     double* d_scratch_flux = nullptr;
     size_t scratch_pixels = 0;
@@ -98,7 +100,12 @@ static int validate(const raptor_params* p) {
     if (p->max_steps < 1) return fail(nullptr, RAPTOR_EINVAL, "max_steps must be >= 1");
     if (!(p->r_stop_in_factor > 0.0) || !(p->r_stop_out_factor >= 1.0)) return fail(nullptr, RAPTOR_EINVAL, "bad r_stop factors");
     if (std::isnan(p->tau_cutoff)) return fail(nullptr, RAPTOR_EINVAL, "tau_cutoff is NaN");
-    if (p->plasma_model < 0 || p->plasma_model > 5) return fail(nullptr, RAPTOR_EINVAL, "unknown plasma_model %d", p->plasma_model);
+    if (p->plasma_model < 0 || p->plasma_model > 6) return fail(nullptr, RAPTOR_EINVAL, "unknown plasma_model %d", p->plasma_model);
+    if (p->plasma_model == RAPTOR_DISK) {
+        if (p->n_freq != 1) return fail(nullptr, RAPTOR_EINVAL, "DISK: n_freq must be 1 (the line is monochromatic in the emitter frame)");
+        if (!(p->model[1] > 0.0) || !(p->model[2] >= 1.0) || !std::isfinite(p->model[3]))
+            return fail(nullptr, RAPTOR_EINVAL, "DISK: model = [r_in (<= 0: ISCO), r_out > 0, max_order >= 1, p]");
+    }
     if (p->k2_mode != 0 && p->k2_mode != 1) return fail(nullptr, RAPTOR_EINVAL, "k2_mode %d: 0 (K2 = 2 Theta^2, PAPER.md:303) or 1 (exact K2)", p->k2_mode);
     if (p->te_model != 0 && p->te_model != 1) return fail(nullptr, RAPTOR_EINVAL, "te_model %d: 0 (constant T_p/T_e) or 1 (Eq. 47)", p->te_model);
     if (p->te_model == 1 && !(p->model[0] >= 0.0 && p->model[1] >= 0.0)) return fail(nullptr, RAPTOR_EINVAL, "te_model 1 needs model[0] = R_low >= 0, model[1] = R_high >= 0");
@@ -118,6 +125,14 @@ static int validate(const raptor_params* p) {
         if (!(p->gamma_ad > 1.0) || !(p->tp_over_te >= 0.0)) return fail(nullptr, RAPTOR_EINVAL, "gamma_ad > 1, tp_over_te >= 0");
     }
     return RAPTOR_OK;
+}
+
+// innermost stable circular orbit of the equatorial Kerr geodesics (Bardeen, Press & Teukolsky 1972)
+static double r_isco(double a) {
+    const double z1 = 1.0 + std::cbrt(1.0 - a * a) * (std::cbrt(1.0 + a) + std::cbrt(1.0 - a));
+    const double z2 = std::sqrt(3.0 * a * a + z1 * z1);
+    const double sg = a > 0.0 ? 1.0 : (a < 0.0 ? -1.0 : 0.0);
+    return 3.0 + z2 - sg * std::sqrt((3.0 - z1) * (3.0 + z1 + 2.0 * z2));
 }
 
 static void build_kp(raptor_ctx* c) {
@@ -146,6 +161,7 @@ static void build_kp(raptor_ctx* c) {
     k.thetae_scale = (kMP / kME) * (p.gamma_ad - 1.0) / (1.0 + p.tp_over_te);
     k.thetae_num = (kMP / kME) * (p.gamma_ad - 1.0); k.gm1 = p.gamma_ad - 1.0; k.te_model = p.te_model;
     for (int i = 0; i < 16; ++i) k.model[i] = p.model[i];
+    k.disk_r_in = p.model[0] > 0.0 ? p.model[0] : r_isco(p.a);
     if (p.n1 > 0) {
         const double d1 = (p.x1_max - p.x1_min) / p.n1;
         k.x1_first = p.x1_min + 0.5 * d1; k.inv_d1 = 1.0 / d1;
@@ -237,6 +253,38 @@ extern "C" int raptor_render(raptor_ctx* ctx, double* d_image, int32_t* d_status
     O.image = d_image; O.status = d_status; O.nsteps = d_nsteps;
     if (O.ntiles == 0) return RAPTOR_OK;
     return run_rays(ctx, O, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int raptor_render_disk(raptor_ctx* ctx, double* d_image, double* d_redshift, int32_t* d_status, int32_t* d_nsteps,
+                                  void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (ctx->p.plasma_model != RAPTOR_DISK) return fail(ctx, RAPTOR_EINVAL, "raptor_render_disk needs plasma_model = RAPTOR_DISK");
+    if (!d_image || !d_redshift) return fail(ctx, RAPTOR_EINVAL, "NULL buffer");
+    RenderOut O;
+    std::memset(&O, 0, sizeof(O));
+    const unsigned all_tiles = (unsigned)(((ctx->p.nx + 7) / 8) * ((ctx->p.ny + 3) / 4));
+    O.tile_offset = (unsigned)ctx->shard_rank; O.tile_stride = (unsigned)ctx->shard_world;
+    O.ntiles = all_tiles > O.tile_offset ? (all_tiles - O.tile_offset + O.tile_stride - 1) / O.tile_stride : 0;
+    O.image = d_image; O.tau = d_redshift; O.status = d_status; O.nsteps = d_nsteps;
+    if (O.ntiles == 0) return RAPTOR_OK;
+    return run_rays(ctx, O, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int raptor_line_profile(raptor_ctx* ctx, const double* d_image, const double* d_redshift, int32_t nbins, double g_min,
+                                   double g_max, double* d_hist, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (!d_image || !d_redshift || !d_hist) return fail(ctx, RAPTOR_EINVAL, "NULL buffer");
+    if (nbins < 1 || nbins > 65535 || !(g_max > g_min)) return fail(ctx, RAPTOR_EINVAL, "need 1 <= nbins <= 65535 and g_max > g_min");
+    const size_t npix = (size_t)ctx->p.nx * ctx->p.ny;
+    if (ctx->profile_bins < nbins) {
+        if (ctx->d_profile_partial) cudaFree(ctx->d_profile_partial);
+        ctx->d_profile_partial = nullptr; ctx->profile_bins = 0;
+        CK(ctx, cudaMalloc(&ctx->d_profile_partial, sizeof(double) * nbins * (size_t)flux_chunks(npix)));
+        ctx->profile_bins = nbins;
+    }
+    const double area = (ctx->p.fov_M / ctx->p.nx) * (ctx->p.fov_M / ctx->p.ny);
+    CK(ctx, launch_profile(d_image, d_redshift, npix, nbins, g_min, g_max, area, ctx->d_profile_partial, d_hist, (cudaStream_t)cuda_stream));
+    return RAPTOR_OK;
 }
 
 extern "C" int raptor_set_shard(raptor_ctx* ctx, int32_t rank, int32_t world) {
@@ -370,7 +418,7 @@ extern "C" int raptor_fp64_peak(int32_t iters, double* tflops, double* ms) {
 extern "C" int raptor_destroy(raptor_ctx* ctx) {
     if (!ctx) return RAPTOR_OK;
     cudaFree(ctx->d_grid); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_counters);
-    cudaFree(ctx->d_partial); cudaFree(ctx->d_scratch_image); cudaFree(ctx->d_scratch_flux);
+    cudaFree(ctx->d_partial); cudaFree(ctx->d_profile_partial); cudaFree(ctx->d_scratch_image); cudaFree(ctx->d_scratch_flux);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     delete ctx;
     return RAPTOR_OK;

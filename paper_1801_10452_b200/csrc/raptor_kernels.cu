@@ -46,7 +46,7 @@ cudaError_t launch_render(const KP& P, int model, const RenderOut& O, int sm_cou
         break;
     switch (model) {
         RAPTOR_CASE_M(M_VACUUM) RAPTOR_CASE_M(M_SPHERE) RAPTOR_CASE_M(M_TORUS)
-        RAPTOR_CASE_M(M_GRID2D) RAPTOR_CASE_M(M_GRID3DT) RAPTOR_CASE_M(M_SLAB)
+        RAPTOR_CASE_M(M_GRID2D) RAPTOR_CASE_M(M_GRID3DT) RAPTOR_CASE_M(M_SLAB) RAPTOR_CASE_M(M_DISK)
     }
     return cudaErrorInvalidValue;
 }
@@ -88,6 +88,45 @@ __global__ void __launch_bounds__(32) k_flux_final(const double* __restrict__ pa
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
     if (threadIdx.x == 0) flux[k] = acc * scale;
+}
+
+// Line profile of the thin disk (Fig. 6): bin b of [g_min, g_max) collects I of the pixels whose
+// redshift factor falls into it.  Same fixed chunking and tree as the flux => bit-reproducible.
+__global__ void __launch_bounds__(kFluxThreads) k_profile_partial(const double* __restrict__ image, const double* __restrict__ red,
+                                                                  size_t npix, double g_min, double inv_dg, int nbins,
+                                                                  double* __restrict__ partial, int nchunks) {
+    __shared__ double sh[kFluxThreads];
+    const int b = blockIdx.y, chunk = blockIdx.x;
+    const size_t lo = (size_t)chunk * kFluxChunk;
+    const size_t hi = lo + kFluxChunk < npix ? lo + kFluxChunk : npix;
+    double acc = 0.0;
+    for (size_t i = lo + threadIdx.x; i < hi; i += kFluxThreads) {
+        const double g = red[i];
+        if (g > 0.0 && floor((g - g_min) * inv_dg) == (double)b) acc += image[i];
+    }
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = kFluxThreads / 2; o >= 32; o >>= 1) {
+        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x < 32) {
+        double v = sh[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) partial[(size_t)b * nchunks + chunk] = v;
+    }
+}
+
+cudaError_t launch_profile(const double* d_image, const double* d_red, size_t npix, int nbins, double g_min, double g_max,
+                           double scale, double* d_partial, double* d_hist, cudaStream_t stream) {
+    const int nchunks = flux_chunks(npix);
+    const double inv_dg = (double)nbins / (g_max - g_min);
+    k_profile_partial<<<dim3(nchunks, nbins), kFluxThreads, 0, stream>>>(d_image, d_red, npix, g_min, inv_dg, nbins, d_partial, nchunks);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    k_flux_final<<<nbins, 32, 0, stream>>>(d_partial, nchunks, scale, d_hist);
+    return cudaGetLastError();
 }
 
 int flux_chunks(size_t npix) { return (int)((npix + kFluxChunk - 1) / kFluxChunk); }

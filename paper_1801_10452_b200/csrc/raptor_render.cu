@@ -44,7 +44,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
     if (MULTI) {
         for (int k = 0; k < P.n_freq; ++k) { sI[k * sstride] = 0.0; sTau[k * sstride] = 0.0; }
     }
-    int n = 0, ns = 0, st = S_RUNNING;
+    int n = 0, ns = 0, ncross = 0, st = S_RUNNING;
     Geom G;
     { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
     for (;;) {
@@ -61,6 +61,8 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         }
         const double h = step_size(P, G, X[2], K[1], K[2], K[3]);
         const double dl = -h;                                                  // backward [A2]
+        double x1p = 0.0, x2p = 0.0, Kp[4] = {0.0, 0.0, 0.0, 0.0};             // thin disk: state before the step
+        if (MODEL == M_DISK) { x1p = X[1]; x2p = X[2]; Kp[0] = K[0]; Kp[1] = K[1]; Kp[2] = K[2]; Kp[3] = K[3]; }
         const double hl = 0.5 * dl;
         Geom Gs;                        // geometry of the last stage point: the new base point is reached from it
         double t1, t2;                  // new point minus that stage point (x1, x2)
@@ -154,6 +156,15 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         if ((n & RAPTOR_REFRESH) == 0) { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
         else if (INTEG == I_VERLET || INTEG == I_VERLET_C) G = Gs;
         else geom_shift<H1>(P, Gs, X[1], X[2], t1, t2, G);
+        if (MODEL == M_DISK) {
+            // I = sum of g^p / r^2 over the counted crossings, tau = g of the first counted one
+            double dI, gg;
+            bool counted;
+            if (disk_crossing(P, x1p, x2p, Kp, X, K, ncross + 1, dI, gg, counted)) {
+                ++ncross;
+                if (counted) { I += dI; if (ns == 0) tau = gg; ++ns; }
+            }
+        } else
         if (MODEL != M_VACUUM && G.r >= P.r_in && G.r <= P.r_out) {            // [A8] end-point sample
             Plasma pl;
             if (plasma_sample<MODEL>(P, G, X, K[0], G.ex * K[1], G.dth * K[2], K[3], pl)) {
@@ -294,7 +305,7 @@ RAPTOR_INST(RAPTOR_MODEL, RAPTOR_INTEG)
 #else
 #define RAPTOR_INST_ALL(M) RAPTOR_INST(M, I_RK4) RAPTOR_INST(M, I_VERLET) RAPTOR_INST(M, I_VERLET_C) RAPTOR_INST(M, I_RK2)
 RAPTOR_INST_ALL(M_VACUUM) RAPTOR_INST_ALL(M_SPHERE) RAPTOR_INST_ALL(M_TORUS)
-RAPTOR_INST_ALL(M_GRID2D) RAPTOR_INST_ALL(M_GRID3DT) RAPTOR_INST_ALL(M_SLAB)
+RAPTOR_INST_ALL(M_GRID2D) RAPTOR_INST_ALL(M_GRID3DT) RAPTOR_INST_ALL(M_SLAB) RAPTOR_INST_ALL(M_DISK)
 #endif
 
 }  // namespace raptor

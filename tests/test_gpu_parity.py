@@ -339,3 +339,62 @@ def test_electron_temperature_eq47_parity(rb, orc, r_low, r_high):
     check_full(rb, orc, replace(scenes.config_C4(nx=24, n1=48, n2=32, n3=16, nt=8), te_model=1, model=model))
     base = gpu_render(rb, scenes.config_C2(nx=40))
     assert abs(g["flux"][0] / base["flux"][0] - 1.0) > 1e-3        # the option does something
+
+
+# ------------------------------------------------- 8(f) f3: thin-disk workload (Sect. 4.2.1)
+def gpu_render_disk(rb, scene, bins=None):
+    with rb.Raptor(scene) as R:
+        image, red, status, nsteps = R.render_disk()
+        hist = R.line_profile(image, red, *bins).cpu().numpy() if bins else None
+        torch.cuda.synchronize()
+        return dict(image=image.cpu().numpy(), redshift=red.cpu().numpy(), status=status.cpu().numpy(),
+                    nsteps=nsteps.cpu().numpy(), hist=hist, counters=R.counters())
+
+
+@pytest.mark.parametrize("a,incl,order,h", [(0.0, 60.0, 1, 1.0), (0.9375, 75.0, 10, 1.0), (-0.5, 40.0, 3, 0.3),
+                                             (0.99, 85.0, 10, 0.3)])
+def test_thin_disk_image_redshift_and_line_profile(rb, orc, a, incl, order, h):
+    s = replace(scenes.thin_disk(a=a, incl_deg=incl, nx=64, max_order=order, mks_h=h), ny=40)
+    bins = (50, 0.0, 1.6)
+    g = gpu_render_disk(rb, s, bins)
+    o = orc.Oracle(s)
+    ref = o.render_disk()
+    keep = ~ring_mask(s)
+    assert (g["status"][keep] == ref["status"][keep]).all() and (g["nsteps"][keep] == ref["nsteps"][keep]).all()
+    # the set of pixels that see the disk is an integer decision: identical outside the ring band, except where a
+    # crossing radius sits within round-off of the disk's edges (none on these grids)
+    assert ((g["redshift"] > 0) == (ref["redshift"][0] > 0))[keep].all()
+    assert (rel_err(g["image"][None], ref["image"])[0][keep] <= 1e-8).mean() >= 0.999
+    m = keep & (ref["redshift"][0] > 0)
+    assert np.abs(g["redshift"][m] / ref["redshift"][0][m] - 1.0).max() <= 1e-9
+    assert g["counters"][1] == ref["sampled"] or abs(g["counters"][1] - ref["sampled"]) <= 10 * int((~keep).sum()) + 2
+    # line profile: the GPU histogram of the GPU image equals numpy's histogram of the same image (same binning
+    # rule, fixed summation order on the GPU: agreement to round-off), and the oracle's to bin-edge flips
+    gg, II = g["redshift"].ravel(), g["image"].ravel()
+    area = (s.fov_M / s.nx) * (s.fov_M / s.ny)
+    sel = gg > 0
+    idx = np.floor((gg[sel] - bins[1]) * (bins[0] / (bins[2] - bins[1]))).astype(int)
+    ok = (idx >= 0) & (idx < bins[0])
+    ref_hist = np.bincount(idx[ok], weights=II[sel][ok] * area, minlength=bins[0])
+    assert np.allclose(g["hist"], ref_hist, rtol=1e-12, atol=1e-300)
+    oh = o.line_profile(ref["image"], ref["redshift"], *bins)
+    assert abs(g["hist"].sum() - oh.sum()) <= 1e-6 * oh.sum()
+    assert np.abs(np.cumsum(g["hist"]) - np.cumsum(oh)).max() <= 2e-3 * oh.sum()
+
+
+def test_thin_disk_full_size_sampled(rb, orc):
+    s = scenes.thin_disk(a=0.5, incl_deg=70.0, nx=512, max_order=10)
+    g = gpu_render_disk(rb, s)
+    o = orc.Oracle(s)
+    ring = ring_mask(s)
+    rng = np.random.default_rng(6)
+    used = 0
+    for x, y in zip(rng.integers(96, 416, 80), rng.integers(160, 352, 80)):
+        if ring[y, x]:
+            continue
+        used += 1
+        r = o.trace(*o.pixel_ab(x, y))
+        assert g["nsteps"][y, x] == r["nsteps"]
+        assert abs(g["image"][y, x] - r["I"][0]) <= 1e-8 * abs(r["I"][0]) + 1e-300, (x, y)
+        assert abs(g["redshift"][y, x] - r["tau"][0]) <= 1e-9 * abs(r["tau"][0]) + 1e-300
+    assert used > 50 and (g["image"] > 0).mean() > 0.2
