@@ -126,6 +126,21 @@ int raptor_render_disk(raptor_ctx *ctx, double *d_image, double *d_redshift, int
 int raptor_line_profile(raptor_ctx *ctx, const double *d_image, const double *d_redshift, int32_t nbins, double g_min,
                         double g_max, double *d_hist, void *cuda_stream);
 
+/* Slow-light movies and light curves (Sect. 5; plasma_model = RAPTOR_GRID3DT, slow_light = 1).
+ * The context holds nt snapshots; for a series longer than nt they form a sliding window: snapshot m (time
+ * t0 + m dt_snap) lives in slot m mod nt, and the resident window is [first, first + nt).  A ray's coordinate time
+ * is clamped to the window.  raptor_upload_snapshot copies ONE snapshot (host, [n1][n2][n3][8]) into its slot on the
+ * stream; raptor_set_window moves the window (default first = 0); raptor_set_camera_time changes t_cam (the
+ * time-calibration delay of Sect. 5.1, is part of t_cam [A15]). */
+int raptor_set_camera_time(raptor_ctx *ctx, double t_cam);
+int raptor_set_window(raptor_ctx *ctx, int64_t first_snapshot);
+int raptor_upload_snapshot(raptor_ctx *ctx, int64_t snapshot, const void *snapshot_host, uint64_t bytes, void *cuda_stream);
+
+/* Light curve: frames f = 0 .. n_frames-1 rendered at camera times t_cam0 + f dt_frame through the resident window
+ * and reduced to d_flux_jy[f][k] (device, [n_frames][n_freq], Jy); the images are not kept.  The context's own
+ * t_cam is left unchanged. */
+int raptor_light_curve(raptor_ctx *ctx, int32_t n_frames, double t_cam0, double dt_frame, double *d_flux_jy, void *cuda_stream);
+
 /* Multi-GPU sharding of one image: after this call raptor_render / raptor_spectrum /
  * raptor_render_host trace only the 8x4-pixel tiles rank, rank + world, rank + 2 world, ... (row-major tile
  * order) and leave every other pixel of the output buffers untouched.  Rays are independent, so the ranks'

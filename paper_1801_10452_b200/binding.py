@@ -22,7 +22,8 @@ STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 
 
 # every symbol include/raptor.h declares
 SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_render_disk",
-           "raptor_line_profile", "raptor_spectrum", "raptor_flux",
+           "raptor_line_profile", "raptor_set_camera_time", "raptor_set_window", "raptor_upload_snapshot",
+           "raptor_light_curve", "raptor_spectrum", "raptor_flux",
            "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_get_counters", "raptor_fp64_peak",
            "raptor_destroy", "raptor_last_error")
 
@@ -69,6 +70,10 @@ def lib():
         L.raptor_upload_grid.argtypes = [vp, vp, C.c_uint64, vp]
         L.raptor_set_shard.argtypes = [vp, i32, i32]
         L.raptor_render.argtypes = [vp, vp, vp, vp, vp]
+        L.raptor_set_camera_time.argtypes = [vp, C.c_double]
+        L.raptor_set_window.argtypes = [vp, C.c_int64]
+        L.raptor_upload_snapshot.argtypes = [vp, C.c_int64, vp, C.c_uint64, vp]
+        L.raptor_light_curve.argtypes = [vp, i32, C.c_double, C.c_double, vp, vp]
         L.raptor_render_disk.argtypes = [vp, vp, vp, vp, vp, vp]
         L.raptor_line_profile.argtypes = [vp, vp, vp, i32, C.c_double, C.c_double, vp, vp]
         L.raptor_spectrum.argtypes = [vp, vp, vp, vp]
@@ -141,6 +146,22 @@ def raptor_render_disk(ctx, d_image, d_redshift, d_status=None, d_nsteps=None, s
 
 def raptor_line_profile(ctx, d_image, d_redshift, nbins, g_min, g_max, d_hist, stream=None):
     _check(lib().raptor_line_profile(ctx, d_image, d_redshift, int(nbins), float(g_min), float(g_max), d_hist, stream), ctx)
+
+
+def raptor_set_camera_time(ctx, t_cam):
+    _check(lib().raptor_set_camera_time(ctx, float(t_cam)), ctx)
+
+
+def raptor_set_window(ctx, first_snapshot):
+    _check(lib().raptor_set_window(ctx, int(first_snapshot)), ctx)
+
+
+def raptor_upload_snapshot(ctx, snapshot, h_snapshot, nbytes, stream=None):
+    _check(lib().raptor_upload_snapshot(ctx, int(snapshot), h_snapshot, nbytes, stream), ctx)
+
+
+def raptor_light_curve(ctx, n_frames, t_cam0, dt_frame, d_flux, stream=None):
+    _check(lib().raptor_light_curve(ctx, int(n_frames), float(t_cam0), float(dt_frame), d_flux, stream), ctx)
 
 
 def raptor_set_shard(ctx, rank, world):
@@ -240,6 +261,25 @@ class Raptor:
         hist = torch.empty((int(nbins),), dtype=torch.float64, device="cuda")
         raptor_line_profile(self.ctx, image.data_ptr(), redshift.data_ptr(), nbins, g_min, g_max, hist.data_ptr(), _stream_ptr())
         return hist
+
+    def light_curve(self, n_frames, t_cam0, dt_frame):
+        """Fluxes [n_frames][n_freq] (CUDA tensor, Jy) of frames at camera times t_cam0 + f dt_frame."""
+        import torch
+        flux = torch.empty((int(n_frames), self.nf), dtype=torch.float64, device="cuda")
+        raptor_light_curve(self.ctx, n_frames, t_cam0, dt_frame, flux.data_ptr(), _stream_ptr())
+        return flux
+
+    def upload_snapshot(self, index, snapshot):
+        g = np.ascontiguousarray(snapshot, dtype=np.float32 if self.scene.grid_dtype == 1 else np.float64)
+        raptor_upload_snapshot(self.ctx, index, g.ctypes.data, g.nbytes, None)
+        import torch
+        torch.cuda.synchronize()
+
+    def set_window(self, first_snapshot):
+        raptor_set_window(self.ctx, first_snapshot)
+
+    def set_camera_time(self, t_cam):
+        raptor_set_camera_time(self.ctx, t_cam)
 
     def set_shard(self, rank, world):
         raptor_set_shard(self.ctx, rank, world)

@@ -12,11 +12,15 @@
 
 using namespace raptor;
 
+struct raptor_ctx;
+static int ensure_scratch(raptor_ctx* ctx);
+
 struct raptor_ctx {
     raptor_params p;
     KP kp;
     int device = 0, sm_count = 148;
     int shard_rank = 0, shard_world = 1;   // raptor_set_shard
+    long long window_lo = 0;               // raptor_set_window
     void* d_grid = nullptr;
     size_t grid_bytes = 0;
     double* d_freq = nullptr;
@@ -285,6 +289,51 @@ extern "C" int raptor_line_profile(raptor_ctx* ctx, const double* d_image, const
     const double area = (ctx->p.fov_M / ctx->p.nx) * (ctx->p.fov_M / ctx->p.ny);
     CK(ctx, launch_profile(d_image, d_redshift, npix, nbins, g_min, g_max, area, ctx->d_profile_partial, d_hist, (cudaStream_t)cuda_stream));
     return RAPTOR_OK;
+}
+
+// ---- slow-light movies and light curves (Sect. 5) -----------------------------------------
+extern "C" int raptor_set_camera_time(raptor_ctx* ctx, double t_cam) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (!std::isfinite(t_cam)) return fail(ctx, RAPTOR_EINVAL, "t_cam must be finite");
+    ctx->p.t_cam = t_cam; ctx->kp.t_cam = t_cam;
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_set_window(raptor_ctx* ctx, int64_t first_snapshot) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (ctx->p.plasma_model != RAPTOR_GRID3DT) return fail(ctx, RAPTOR_EINVAL, "raptor_set_window needs plasma_model = RAPTOR_GRID3DT");
+    if (first_snapshot < 0 || first_snapshot > (1ll << 40)) return fail(ctx, RAPTOR_EINVAL, "first_snapshot out of range");
+    ctx->window_lo = first_snapshot;
+    ctx->kp.snap_lo = (double)first_snapshot;
+    ctx->kp.snap_lo_mod = (int)(first_snapshot % ctx->p.nt);
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_upload_snapshot(raptor_ctx* ctx, int64_t snapshot, const void* host, uint64_t bytes, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (ctx->p.plasma_model != RAPTOR_GRID3DT || !ctx->d_grid) return fail(ctx, RAPTOR_EINVAL, "raptor_upload_snapshot needs plasma_model = RAPTOR_GRID3DT");
+    const size_t one = ctx->grid_bytes / (size_t)ctx->p.nt;
+    if (!host || bytes != one) return fail(ctx, RAPTOR_EINVAL, "snapshot bytes %llu != n1*n2*n3*8*elem = %zu", (unsigned long long)bytes, one);
+    if (snapshot < 0) return fail(ctx, RAPTOR_EINVAL, "snapshot index < 0");
+    const size_t slot = (size_t)(snapshot % ctx->p.nt);
+    CK(ctx, cudaMemcpyAsync((char*)ctx->d_grid + slot * one, host, one, cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream));
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_light_curve(raptor_ctx* ctx, int32_t n_frames, double t_cam0, double dt_frame, double* d_flux_jy, void* cuda_stream) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (n_frames < 0 || (n_frames > 0 && !d_flux_jy)) return fail(ctx, RAPTOR_EINVAL, "n_frames < 0 or d_flux_jy NULL");
+    if (!std::isfinite(t_cam0) || !std::isfinite(dt_frame)) return fail(ctx, RAPTOR_EINVAL, "t_cam0, dt_frame must be finite");
+    int rc = ensure_scratch(ctx);
+    if (rc) return rc;
+    const double keep = ctx->kp.t_cam;
+    for (int f = 0; f < n_frames && !rc; ++f) {
+        ctx->kp.t_cam = t_cam0 + (double)f * dt_frame;
+        rc = raptor_render(ctx, ctx->d_scratch_image, nullptr, nullptr, cuda_stream);
+        if (!rc) rc = raptor_flux(ctx, ctx->d_scratch_image, d_flux_jy + (size_t)f * ctx->p.n_freq, cuda_stream);
+    }
+    ctx->kp.t_cam = keep;
+    return rc;
 }
 
 extern "C" int raptor_set_shard(raptor_ctx* ctx, int32_t rank, int32_t world) {

@@ -398,3 +398,33 @@ def test_thin_disk_full_size_sampled(rb, orc):
         assert abs(g["image"][y, x] - r["I"][0]) <= 1e-8 * abs(r["I"][0]) + 1e-300, (x, y)
         assert abs(g["redshift"][y, x] - r["tau"][0]) <= 1e-9 * abs(r["tau"][0]) + 1e-300
     assert used > 50 and (g["image"] > 0).mean() > 0.2
+
+
+# ------------------------------------------------- 8(f) f4: light curves through a sliding snapshot window
+def test_light_curve_sliding_window_parity(rb, orc):
+    from paper_1801_10452_b200 import lightcurve
+    series = scenes.config_C4(nx=16, n1=32, n2=24, n3=16, nt=24)          # 24 snapshots, t = 0 .. 230 M
+    nt, n_snap = 8, 24
+    s = replace(series, nt=nt, grid=series.grid[:nt], freq_hz=(43e9, 230e9), snapshot=0)
+    t_cams = [scenes.slow_light_t_cam(1000.0, t_mid) for t_mid in (35.0, 62.0, 130.0, 200.0, 118.0)]
+    with rb.Raptor(s) as R:
+        F = lightcurve.render_light_curve(R, t_cams, series=lambda m: series.grid[m], n_snap=n_snap)
+        # the multi-frame C-ABI call on the window the last frame left resident
+        lo_last = lightcurve.window_start(t_cams[-1], s.r_cam, s.t0, s.dt_snap, nt, n_snap)
+        F2 = R.light_curve(3, t_cams[-1] - 7.0, 7.0).cpu().numpy()
+    assert F.shape == (5, 2) and np.isfinite(F).all() and (F > 0).all()
+    los = []
+    for f, tc in enumerate(t_cams):
+        lo = lightcurve.window_start(tc, s.r_cam, s.t0, s.dt_snap, nt, n_snap)
+        los.append(lo)
+        so = replace(s, grid=series.grid[lo:lo + nt], t0=lo * s.dt_snap, t_cam=tc)
+        o = orc.Oracle(so)
+        ref = o.flux(o.render()["image"])
+        assert np.abs(F[f] / ref - 1.0).max() <= 1e-9, (f, lo, F[f], ref)
+    assert len(set(los)) >= 3 and max(los) > nt                          # the window really moved and wrapped
+    assert np.abs(F2[1] / F[-1] - 1.0).max() <= 1e-13
+    for j, dt in enumerate((-7.0, 0.0, 7.0)):
+        so = replace(s, grid=series.grid[lo_last:lo_last + nt], t0=lo_last * s.dt_snap, t_cam=t_cams[-1] + dt)
+        o = orc.Oracle(so)
+        assert np.abs(F2[j] / o.flux(o.render()["image"]) - 1.0).max() <= 1e-9
+    assert np.ptp(F[:, 1]) / F[:, 1].mean() > 1e-3                        # the source varies in time
