@@ -300,6 +300,17 @@ def slab_scene(n_e: float, theta_e: float, B_gauss: float, thickness_M: float,
     return Scene(**base)
 
 
+def config_PB1(nx: int = 512, n1: int = 256, n2: int = 256) -> Scene:
+    """The paper's own performance configuration (Table B.1): 512 x 512 pixels, image size 40 M,
+    step rule Eq. 21-24 with eps = 0.03, integration scheme "RK2" (midpoint [A17]), radiative transfer on; camera,
+    frequency, inclination, tau cut-off and T_p/T_e from Table 2: r_cam = 1e4 M, 230 GHz,
+    i = 90 deg, tau_cutoff = ln 1000, T_p/T_e = 3.  The BHAC dump is replaced by the seeded 2-D grid of C2; FP64
+    instead of the paper's single precision."""
+    base = config_C2(nx=nx, n1=n1, n2=n2)
+    return replace(base, name="PB1", incl_deg=90.0, r_cam=1.0e4, integrator=3, step_policy=1, eps=0.03,
+                   tau_cutoff=math.log(1000.0), tp_over_te=3.0)
+
+
 def thin_disk(a: float = 0.0, incl_deg: float = 60.0, nx: int = 256, r_out: float = 15.0, max_order: int = 10,
               p: float = 3.0, r_in: float = 0.0, **kw) -> Scene:
     """Thin-disk workload of Sect. 4.2.1: equatorial Keplerian disk from the ISCO (r_in <= 0)
@@ -311,7 +322,7 @@ def thin_disk(a: float = 0.0, incl_deg: float = 60.0, nx: int = 256, r_out: floa
     return Scene(**base)
 
 
-CONFIGS = {"C0": config_C0, "C1": config_C1, "C2": config_C2, "C3": config_C3, "C4": config_C4}
+CONFIGS = {"C0": config_C0, "C1": config_C1, "C2": config_C2, "C3": config_C3, "C4": config_C4, "PB1": config_PB1}
 
 
 def config(name: str, **kw) -> Scene:
