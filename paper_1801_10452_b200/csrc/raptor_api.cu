@@ -144,6 +144,7 @@ static void build_kp(raptor_ctx* c) {
     KP& k = c->kp;
     std::memset(&k, 0, sizeof(k));
     k.a = p.a; k.a2 = p.a * p.a; k.twoa = 2.0 * p.a; k.m = p.mass; k.twom = 2.0 * p.mass; k.omh = 1.0 - p.mks_h; k.r0 = p.mks_r0;
+    k.pi_omh = kPI * k.omh; k.half_omh = 0.5 * k.omh; k.d2th_c = (-2.0 * kPI * kPI) * k.omh;
     const double inc = p.incl_deg * (kPI / 180.0);
     k.r_cam = p.r_cam; k.sin_i = std::sin(inc); k.cos_i = std::cos(inc);
     k.sq1mc2 = std::sqrt(1.0 - k.cos_i * k.cos_i);
@@ -156,6 +157,7 @@ static void build_kp(raptor_ctx* c) {
     k.eps = p.eps; k.delta = p.delta; k.eps_polar = p.eps_polar;
     const double disc = p.mass * p.mass - p.a * p.a;
     k.rH = disc >= 0.0 ? p.mass + std::sqrt(disc) : 0.0;
+    k.step_c_rH = -p.step_c * k.rH;
     k.r_in = p.r_stop_in_factor * k.rH; k.r_out = p.r_stop_out_factor * p.r_cam;
     k.tau_cutoff = p.tau_cutoff; k.use_tau_cutoff = std::isfinite(p.tau_cutoff) ? 1 : 0;
     k.Lcm = kG * p.M_bh_g / (kC * kC);
