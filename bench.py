@@ -34,12 +34,18 @@ UNIT = "steps/s"
 # lanes x 2 flop x 1.965 GHz (clocks.max.sm).  The live DFMA probe (raptor_fp64_peak) is reported beside it.
 FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
 
-# FP64 flop per accepted RK4 step of each workload: thread-level executed DFMA x 2 +
-# DMUL + DADD of the shipped k_render kernel divided by the accepted steps, counted with ncu
-# (profiles/flop_per_step_r1.md).  It contains the 4 RHS evaluations with their exp / sin / cos, the RK4
-# combination and the sampled steps' share of sampler + transfer arithmetic.  Integer and control
-# instructions are not counted.  C3's figure is for its 32 frequencies.
-FLOP_PER_STEP = {"C0": 1610.9, "C1": 884.7, "C2": 1084.2, "C3": 1507.3, "C4": 1094.2}
+# FP64 work per accepted integrator step of each workload: thread-level executed
+# (DFMA, DMUL, DADD) of the shipped k_render kernel divided by the accepted steps, counted with ncu
+# (profiles/flop_per_step_r1.md).  flop = 2 DFMA + DMUL + DADD.  It contains the RHS evaluations with their
+# exp / sin / cos, the integrator's combination and the sampled steps' share of sampler + transfer arithmetic.
+# Integer and control instructions are not counted.  C3's figure is for its 32 frequencies.
+FP64_INST_PER_STEP = {"C0": (476.5, 335.9, 101.1), "C1": (200.2, 225.1, 20.2), "C2": (235.5, 255.6, 24.7),
+                      "C3": (369.4, 293.3, 39.3), "C4": (245.1, 256.9, 29.1), "PB1": (261.8, 171.9, 32.1)}
+FLOP_PER_STEP = {k: 2.0 * v[0] + v[1] + v[2] for k, v in FP64_INST_PER_STEP.items()}
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_render launch (ncu --set full, profiles/k_render_C2_r1.md)
+DRAM_BYTES_PER_LAUNCH = {"C2": 4.264e6 + 0.035e6}
+# paper's own numbers for its performance configuration (Table B.1 / PAPER.md:342, 666): context for PB1 only
+PAPER_GEODESICS_PER_SEC = {"GTX 1080, OpenACC, single precision": 104900.0, "i7-6950X 10 cores, OpenMP, single precision": 10707.0}
 
 
 def build_scene(workload: str):
@@ -254,6 +260,12 @@ def run_ours(args):
         avg_render_ms = sum(render_ms) / len(render_ms)
         flops_launch = algorithmic_flops(scene, args.workload, steps_done / args.steps, sampled_done / args.steps)
         achieved = flops_launch / (avg_render_ms * 1e-3) / 1e12
+        # the FP64 pipe issues one warp instruction per 2 cycles per sub-partition whether it is a DFMA or a DMUL/DADD:
+        # share of those issue slots the kernel's DFMA + DMUL + DADD fill, and the flop ceiling its mix allows
+        fi = FP64_INST_PER_STEP[args.workload]
+        n_inst = sum(fi) * steps_done / args.steps
+        pipe_frac = n_inst / (148 * 4 * 16 * 1.965e9 * avg_render_ms * 1e-3)
+        mix_ceiling = FLOP_PER_STEP[args.workload] / (2.0 * sum(fi))
         # CPU baseline: the oracle on a bounded sample of the same workload (about 10-30 s of host work)
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
@@ -281,8 +293,11 @@ def run_ours(args):
             "e2e": {"value": e2e_units_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "images_per_sec": world * e2e_steps / (e2e_ms_max * 1e-3)},
             "gpu_launches": 3 * args.steps,
+            "rays_per_sec": world * args.steps * scene.nx * scene.ny / (total_ms_max * 1e-3),
             "roofline": {"bound": "alu", "kernel": "k_render", "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
-                         "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None,
+                         "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": DRAM_BYTES_PER_LAUNCH.get(args.workload),
+                         "fp64_pipe_frac": pipe_frac, "mix_ceiling": mix_ceiling,
+                         "fp64_inst_per_step": {"dfma": fi[0], "dmul": fi[1], "dadd": fi[2]},
                          "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md)",
                          "fp64_probe_tflops": fp64_probe, "kernel_ms": avg_render_ms,
                          "kernel_share_of_step": avg_render_ms / (total_ms / args.steps),
@@ -290,6 +305,8 @@ def run_ours(args):
             "cpu_baseline": cpu,
             "wall_s_timed_region": t_wall,
         }
+        if args.workload == "PB1":
+            line["paper_geodesics_per_sec"] = PAPER_GEODESICS_PER_SEC      # other hardware, FP32: context only
         print(json.dumps(line))
     R.close()
     if world > 1:
@@ -302,7 +319,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "PB1"])
     ap.add_argument("--ref-row-stride", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
