@@ -137,8 +137,10 @@ int raptor_set_window(raptor_ctx *ctx, int64_t first_snapshot);
 int raptor_upload_snapshot(raptor_ctx *ctx, int64_t snapshot, const void *snapshot_host, uint64_t bytes, void *cuda_stream);
 
 /* Light curve: frames f = 0 .. n_frames-1 rendered at camera times t_cam0 + f dt_frame through the resident window
- * and reduced to d_flux_jy[f][k] (device, [n_frames][n_freq], Jy); the images are not kept.  The context's own
- * t_cam is left unchanged. */
+ * and reduced to d_flux_jy[f][k] (device, [n_frames][n_freq], Jy); the images are not kept.  The frames of a batch
+ * (up to 256 MiB of images) are traced by ONE launch of the ray kernel -- small frames cannot fill the GPU one at a
+ * time -- and reduced by one deterministic reduction.  The context's own t_cam is left unchanged; the tile shard
+ * must be (0, 1) (light curves shard by frames). */
 int raptor_light_curve(raptor_ctx *ctx, int32_t n_frames, double t_cam0, double dt_frame, double *d_flux_jy, void *cuda_stream);
 
 /* Multi-GPU sharding of one image: after this call raptor_render / raptor_spectrum /

@@ -1,6 +1,7 @@
 // raptor_api.cu -- the C ABI of include/raptor.h: validation, scene upload, launches.  Host code only.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -28,6 +29,8 @@ struct raptor_ctx {
     unsigned long long* d_counters = nullptr;
     double* d_partial = nullptr;      // flux partial sums [n_freq][chunks]
     double* d_profile_partial = nullptr;   // line-profile partial sums [nbins][chunks]
+    double* d_lc_partial = nullptr;        // light-curve partial sums [frames * n_freq][chunks]
+    size_t lc_planes = 0;
     int profile_bins = 0;
     double* d_scratch_image = nullptr;
     double* d_scratch_flux = nullptr;
@@ -283,7 +286,7 @@ extern "C" int raptor_line_profile(raptor_ctx* ctx, const double* d_image, const
     if (nbins < 1 || nbins > 65535 || !(g_max > g_min)) return fail(ctx, RAPTOR_EINVAL, "need 1 <= nbins <= 65535 and g_max > g_min");
     const size_t npix = (size_t)ctx->p.nx * ctx->p.ny;
     if (ctx->profile_bins < nbins) {
-        if (ctx->d_profile_partial) cudaFree(ctx->d_profile_partial);
+        if (ctx->d_profile_partial) cudaFree(ctx->d_profile_partial); cudaFree(ctx->d_lc_partial);
         ctx->d_profile_partial = nullptr; ctx->profile_bins = 0;
         CK(ctx, cudaMalloc(&ctx->d_profile_partial, sizeof(double) * nbins * (size_t)flux_chunks(npix)));
         ctx->profile_bins = nbins;
@@ -322,20 +325,58 @@ extern "C" int raptor_upload_snapshot(raptor_ctx* ctx, int64_t snapshot, const v
     return RAPTOR_OK;
 }
 
+// frames of a light curve rendered per launch: the image scratch is frames x n_freq x npix doubles
+static const size_t kLightCurveScratchBytes = 256u << 20;
+
 extern "C" int raptor_light_curve(raptor_ctx* ctx, int32_t n_frames, double t_cam0, double dt_frame, double* d_flux_jy, void* cuda_stream) {
     if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
     if (n_frames < 0 || (n_frames > 0 && !d_flux_jy)) return fail(ctx, RAPTOR_EINVAL, "n_frames < 0 or d_flux_jy NULL");
     if (!std::isfinite(t_cam0) || !std::isfinite(dt_frame)) return fail(ctx, RAPTOR_EINVAL, "t_cam0, dt_frame must be finite");
-    int rc = ensure_scratch(ctx);
-    if (rc) return rc;
-    const double keep = ctx->kp.t_cam;
-    for (int f = 0; f < n_frames && !rc; ++f) {
-        ctx->kp.t_cam = t_cam0 + (double)f * dt_frame;
-        rc = raptor_render(ctx, ctx->d_scratch_image, nullptr, nullptr, cuda_stream);
-        if (!rc) rc = raptor_flux(ctx, ctx->d_scratch_image, d_flux_jy + (size_t)f * ctx->p.n_freq, cuda_stream);
+    if (ctx->shard_world != 1) return fail(ctx, RAPTOR_EUNSUPPORTED, "raptor_light_curve shards by frames, not by tiles: reset raptor_set_shard(0, 1)");
+    if (n_frames == 0) return RAPTOR_OK;
+    const raptor_params& p = ctx->p;
+    const size_t npix = (size_t)p.nx * p.ny, per_frame = npix * p.n_freq;
+    size_t batch = kLightCurveScratchBytes / (per_frame * sizeof(double));
+    if (batch < 1) batch = 1;
+    if (batch > (size_t)n_frames) batch = (size_t)n_frames;
+    const unsigned tiles = (unsigned)(((p.nx + 7) / 8) * ((p.ny + 3) / 4));
+    if ((unsigned long long)tiles * batch > 0x7fffffffull) batch = 0x7fffffffull / tiles;
+    if (batch * p.n_freq > 65535) batch = 65535 / p.n_freq;                 // grid.y of the flux reduction
+    // scratch for `batch` images and their flux partial sums
+    if (ctx->scratch_pixels < batch * per_frame) {
+        if (ctx->d_scratch_image) cudaFree(ctx->d_scratch_image);
+        ctx->d_scratch_image = nullptr; ctx->scratch_pixels = 0;
+        CK(ctx, cudaMalloc(&ctx->d_scratch_image, batch * per_frame * sizeof(double)));
+        ctx->scratch_pixels = batch * per_frame;
     }
-    ctx->kp.t_cam = keep;
-    return rc;
+    const size_t planes = batch * p.n_freq;
+    if (ctx->lc_planes < planes) {
+        if (ctx->d_lc_partial) cudaFree(ctx->d_lc_partial);
+        ctx->d_lc_partial = nullptr; ctx->lc_planes = 0;
+        CK(ctx, cudaMalloc(&ctx->d_lc_partial, sizeof(double) * planes * (size_t)flux_chunks(npix)));
+        ctx->lc_planes = planes;
+    }
+    const double L = ctx->kp.Lcm;
+    const double scale = 1e23 * (p.fov_M / p.nx) * (p.fov_M / p.ny) * L * L / (p.D_src_cm * p.D_src_cm);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    for (size_t f0 = 0; f0 < (size_t)n_frames; f0 += batch) {
+        const size_t nb = std::min(batch, (size_t)n_frames - f0);
+        RenderOut O;
+        std::memset(&O, 0, sizeof(O));
+        O.frames = (unsigned)nb; O.tiles_per_frame = tiles; O.ntiles = tiles * (unsigned)nb;
+        O.t_cam0 = t_cam0 + (double)f0 * dt_frame; O.dt_frame = dt_frame;
+        O.image = ctx->d_scratch_image;
+        if (nb == 1) { O.frames = 1; }       // single frame: the ordinary path with its own camera time
+        const double keep = ctx->kp.t_cam;
+        if (nb == 1) ctx->kp.t_cam = O.t_cam0;
+        int rc = run_rays(ctx, O, s);
+        ctx->kp.t_cam = keep;
+        if (rc) return rc;
+        // the batch is [nb][n_freq][npix] = nb * n_freq planes: one deterministic reduction for all of them
+        CK(ctx, launch_flux(ctx->d_scratch_image, npix, (int)(nb * p.n_freq), scale, ctx->d_lc_partial,
+                            d_flux_jy + f0 * p.n_freq, s));
+    }
+    return RAPTOR_OK;
 }
 
 extern "C" int raptor_set_shard(raptor_ctx* ctx, int32_t rank, int32_t world) {
@@ -469,7 +510,7 @@ extern "C" int raptor_fp64_peak(int32_t iters, double* tflops, double* ms) {
 extern "C" int raptor_destroy(raptor_ctx* ctx) {
     if (!ctx) return RAPTOR_OK;
     cudaFree(ctx->d_grid); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_counters);
-    cudaFree(ctx->d_partial); cudaFree(ctx->d_profile_partial); cudaFree(ctx->d_scratch_image); cudaFree(ctx->d_scratch_flux);
+    cudaFree(ctx->d_partial); cudaFree(ctx->d_profile_partial); cudaFree(ctx->d_lc_partial); cudaFree(ctx->d_scratch_image); cudaFree(ctx->d_scratch_flux);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     delete ctx;
     return RAPTOR_OK;

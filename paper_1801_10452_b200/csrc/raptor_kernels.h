@@ -33,6 +33,9 @@ struct RenderOut {
     int32_t* status;                // [npix]
     int32_t* nsteps;                // [npix]
     double* XK;                     // [npix][8] final state
+    unsigned int frames;            // > 1: light-curve batch, image is [frames][n_freq][npix]; ntiles = frames * tiles_per_frame
+    unsigned int tiles_per_frame;
+    double t_cam0, dt_frame;        // camera time of frame f: t_cam0 + f dt_frame
 };
 
 // raptor_render.cu: one explicit instantiation per (plasma model, integrator), one translation unit each

@@ -36,10 +36,11 @@ namespace raptor {
 // (offset dl^2/6 (f_1 - 2 f_2 + f_3)), both of which are second / third order small.
 // --------------------------------------------------------------------------------------------
 template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG>
-__device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta, double* __restrict__ sI,
+__device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta, double t_cam, double* __restrict__ sI,
                                           double* __restrict__ sTau, int sstride, double& I0, double& tau0,
                                           double X[4], double K[4], int& status, int& nsteps, int& nsampled) {
     camera_ray(P, alpha, beta, X, K);
+    X[0] = t_cam;
     double I = 0.0, tau = 0.0;
     if (MULTI) {
         for (int k = 0; k < P.n_freq; ++k) { sI[k * sstride] = 0.0; sTau[k * sstride] = 0.0; }
@@ -217,6 +218,14 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
         if (lane == 0) tile = atomicAdd(O.queue, 1u);
         tile = __shfl_sync(0xffffffffu, tile, 0);
         if (tile >= O.ntiles) break;
+        // light-curve batch: O.frames images of the same scene at camera times t_cam0 + frame dt_frame in one launch
+        unsigned int frame = 0;
+        double t_cam = P.t_cam;
+        if (O.frames > 1) {
+            frame = tile / O.tiles_per_frame;
+            tile -= frame * O.tiles_per_frame;
+            t_cam = fma((double)frame, O.dt_frame, O.t_cam0);
+        }
         tile = O.tile_offset + tile * O.tile_stride;                           // multi-GPU shard: interleaved tiles
         double alpha, beta;
         long long pix;
@@ -237,12 +246,13 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
         if (active) {
             double X[4], K[4], I0, tau0;
             int status, n, ns;
-            trace_ray<MODEL, H1, MULTI, FULLX, INTEG>(P, alpha, beta, sI, sTau, sstride, I0, tau0, X, K, status, n, ns);
+            trace_ray<MODEL, H1, MULTI, FULLX, INTEG>(P, alpha, beta, t_cam, sI, sTau, sstride, I0, tau0, X, K, status, n, ns);
             steps += (unsigned)n; sampled += (unsigned)ns; rays += 1;
             const size_t npix = O.alpha ? (size_t)O.nrays : (size_t)P.nx * P.ny;
             if (O.image) {
-                if (MULTI) { for (int k = 0; k < P.n_freq; ++k) O.image[(size_t)k * npix + pix] = sI[k * sstride]; }
-                else O.image[pix] = I0;
+                double* img = O.image + (size_t)frame * P.n_freq * npix;
+                if (MULTI) { for (int k = 0; k < P.n_freq; ++k) img[(size_t)k * npix + pix] = sI[k * sstride]; }
+                else img[pix] = I0;
             }
             if (O.tau) {
                 if (MULTI) { for (int k = 0; k < P.n_freq; ++k) O.tau[(size_t)k * npix + pix] = sTau[k * sstride]; }
