@@ -40,7 +40,8 @@ FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
 # exp / sin / cos, the integrator's combination and the sampled steps' share of sampler + transfer arithmetic.
 # Integer and control instructions are not counted.  C3's figure is for its 32 frequencies.
 FP64_INST_PER_STEP = {"C0": (476.5, 335.9, 101.1), "C1": (200.2, 225.1, 20.2), "C2": (235.5, 255.6, 24.7),
-                      "C3": (369.4, 293.3, 39.3), "C4": (245.1, 256.9, 29.1), "PB1": (261.8, 171.9, 32.1)}
+                      "C3": (369.4, 293.3, 39.3), "C4": (245.1, 257.1, 30.7), "PB1": (261.8, 171.9, 32.1),
+                      "LC": (257.0, 260.4, 31.9)}
 FLOP_PER_STEP = {k: 2.0 * v[0] + v[1] + v[2] for k, v in FP64_INST_PER_STEP.items()}
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_render launch (ncu --set full, profiles/k_render_C2_r1.md)
 DRAM_BYTES_PER_LAUNCH = {"C2": 4.264e6 + 0.035e6}
@@ -48,8 +49,16 @@ DRAM_BYTES_PER_LAUNCH = {"C2": 4.264e6 + 0.035e6}
 PAPER_GEODESICS_PER_SEC = {"GTX 1080, OpenACC, single precision": 104900.0, "i7-6950X 10 cores, OpenMP, single precision": 10707.0}
 
 
+LC_FRAMES, LC_DT = 32, 2.5      # workload LC: frames per light curve, camera-time spacing [M]
+
+
 def build_scene(workload: str):
     from paper_1801_10452_b200 import scenes
+    if workload == "LC":
+        # slow-light light curve (Sect. 5): 256^2 pixels, the paper's four VLBI frequencies, 16 snapshots
+        from dataclasses import replace
+        s = scenes.config_C4(nx=256, n1=64, n2=48, n3=32, nt=16)
+        return replace(s, name="LC", freq_hz=(22e9, 43e9, 86e9, 230e9))
     return scenes.config(workload)
 
 
@@ -184,8 +193,21 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    lc = args.workload == "LC"
+    lc_flux = torch.empty((LC_FRAMES, scene.n_freq), dtype=torch.float64, device="cuda") if lc else None
+    lc_t0 = scene.t_cam - 0.5 * LC_FRAMES * LC_DT
+
     def one_step(ev=None):
         # a1-a6 + image write (render kernel), a7 flux reduction (2 small kernels): 3 launches
+        if lc:
+            # one light curve: LC_FRAMES frames traced by one k_render launch + one flux reduction over all of them
+            if ev:
+                ev[0].record(stream)
+            binding.raptor_light_curve(R.ctx, LC_FRAMES, lc_t0, LC_DT, lc_flux.data_ptr(), sp)
+            if ev:
+                ev[1].record(stream)
+                ev[2].record(stream)
+            return
         if ev:
             ev[0].record(stream)
         binding.raptor_render(R.ctx, image.data_ptr(), None, None, sp)
@@ -229,9 +251,16 @@ def run_ours(args):
         h_grid = torch.from_numpy(g.reshape(-1).copy()).pin_memory()
     e2e_steps = max(2, min(args.steps, 5))
 
+    h_lc = torch.empty((LC_FRAMES, scene.n_freq), dtype=torch.float64).pin_memory() if lc else None
+
     def e2e_step():
         if h_grid is not None:
             binding.raptor_upload_grid(R.ctx, h_grid.data_ptr(), h_grid.numel() * h_grid.element_size(), None)
+        if lc:
+            binding.raptor_light_curve(R.ctx, LC_FRAMES, lc_t0, LC_DT, lc_flux.data_ptr(), sp)
+            h_lc.copy_(lc_flux, non_blocking=True)
+            torch.cuda.synchronize()
+            return
         binding.raptor_render_host(R.ctx, h_image.data_ptr(), None, None, h_flux.data_ptr())
 
     e2e_step()
@@ -256,7 +285,7 @@ def run_ours(args):
 
     if rank == 0:
         value = steps_all / (total_ms_max * 1e-3)
-        images_per_s = world * args.steps / (total_ms_max * 1e-3)
+        images_per_s = world * args.steps * (LC_FRAMES if lc else 1) / (total_ms_max * 1e-3)
         avg_render_ms = sum(render_ms) / len(render_ms)
         flops_launch = algorithmic_flops(scene, args.workload, steps_done / args.steps, sampled_done / args.steps)
         achieved = flops_launch / (avg_render_ms * 1e-3) / 1e12
@@ -278,7 +307,7 @@ def run_ours(args):
                    "sample": f"every {stride}th row of the {scene.nx}x{scene.ny} {args.workload} image "
                              f"({s} steps in {dt:.1f} s)"}
         h2d = int(h_grid.numel() * h_grid.element_size()) if h_grid is not None else 0
-        d2h = int(h_image.numel() * 8 + h_flux.numel() * 8)
+        d2h = int(h_lc.numel() * 8) if lc else int(h_image.numel() * 8 + h_flux.numel() * 8)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -291,9 +320,10 @@ def run_ours(args):
             "steps_per_image": steps_done / args.steps, "sampled_steps_per_image": sampled_done / args.steps,
             "clocks": clocks,
             "e2e": {"value": e2e_units_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": d2h, "images_per_sec": world * e2e_steps / (e2e_ms_max * 1e-3)},
+                    "d2h_bytes_per_step": d2h, "images_per_sec": world * e2e_steps * (LC_FRAMES if lc else 1) / (e2e_ms_max * 1e-3)},
             "gpu_launches": 3 * args.steps,
-            "rays_per_sec": world * args.steps * scene.nx * scene.ny / (total_ms_max * 1e-3),
+            "frames_per_step": LC_FRAMES if lc else 1,
+            "rays_per_sec": world * args.steps * (LC_FRAMES if lc else 1) * scene.nx * scene.ny / (total_ms_max * 1e-3),
             "roofline": {"bound": "alu", "kernel": "k_render", "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
                          "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": DRAM_BYTES_PER_LAUNCH.get(args.workload),
                          "fp64_pipe_frac": pipe_frac, "mix_ceiling": mix_ceiling,
@@ -319,7 +349,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "PB1"])
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "PB1", "LC"])
     ap.add_argument("--ref-row-stride", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
