@@ -428,3 +428,13 @@ def test_light_curve_sliding_window_parity(rb, orc):
         o = orc.Oracle(so)
         assert np.abs(F2[j] / o.flux(o.render()["image"]) - 1.0).max() <= 1e-9
     assert np.ptp(F[:, 1]) / F[:, 1].mean() > 1e-3                        # the source varies in time
+
+
+# ------------------------------------------------- chart offset r0, negative spin, non-square pixels, near camera
+@pytest.mark.parametrize("cfg", ["C1", "C2"])
+def test_radial_offset_negative_spin_and_rectangular_pixels(rb, orc, cfg):
+    if cfg == "C1":
+        s = replace(scenes.config_C1(64), nx=40, ny=22, a=-0.7, mks_r0=0.6, r_cam=300.0, fov_M=33.0, incl_deg=115.0)
+    else:
+        s = replace(scenes.config_C2(nx=36), ny=20, mks_r0=0.4, r_cam=250.0, incl_deg=140.0)
+    check_full(rb, orc, s)

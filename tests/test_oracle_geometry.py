@@ -270,6 +270,24 @@ def test_P2_mks_chain_rule_same_ray_in_two_charts():
     assert np.allclose(out[0], out[1], rtol=0, atol=2e-9)
 
 
+def test_P2_radial_offset_r0_same_ray_in_two_charts():
+    # r = r0 + exp(x1) (A.10): the same geodesic with r0 = 0 and r0 = 0.5 differs only by truncation,
+    # and negative spin mirrors the image: (a, alpha) -> (-a, -alpha) flips the sign of phi and leaves r, theta, t
+    out = []
+    for r0 in (0.0, 0.5):
+        o = orc.Oracle(vac(a=0.9375, h=0.3, mks_r0=r0, incl_deg=60.0, r_cam=60.0, step_c=0.0, step_min=0.01,
+                           step_max=0.01, eps_polar=1e30, max_steps=8000))
+        res = o.trace(8.0, 4.0)
+        assert res["status"] == 3
+        out.append([res["X"][0], math.log(r0 + math.exp(res["X"][1])), res["X"][2], res["X"][3]])
+    assert np.allclose(out[0], out[1], rtol=0, atol=5e-9)
+    om = orc.Oracle(vac(a=-0.9375, h=0.3, incl_deg=60.0, r_cam=60.0, step_c=0.0, step_min=0.01, step_max=0.01,
+                        eps_polar=1e30, max_steps=8000))
+    rm = om.trace(-8.0, 4.0)
+    assert np.allclose([rm["X"][0], rm["X"][1], rm["X"][2], -rm["X"][3]],
+                       [out[0][0], out[0][1], out[0][2], out[0][3]], rtol=0, atol=1e-11)
+
+
 # ------------------------------------------------------------------------------------- P6
 def _edge(o, direction, lo, hi, tol=2e-6):
     """Bisect along a ray of the image plane for the capture/escape boundary."""
