@@ -170,6 +170,10 @@ int raptor_trace(raptor_ctx *ctx, int32_t n, const double *d_alpha, const double
  * d_XK[n][8] in, d_f[n][4] out (device). */
 int raptor_eval_rhs(raptor_ctx *ctx, int32_t n, const double *d_XK, double *d_f, void *cuda_stream);
 
+/* Diagnostics: the null condition g_mn k^m k^n (Eq. 4) at n states, d_XK[n][8] in (e.g. the final
+ * states raptor_trace returns), d_out[n] out (device).  0 up to the integrator's truncation error. */
+int raptor_null_norm(raptor_ctx *ctx, int32_t n, const double *d_XK, double *d_out, void *cuda_stream);
+
 /* Counters accumulated by every render / trace since creation (synchronises the context's work):
  * accepted RK4 steps, steps on which plasma was sampled, rays traced. */
 int raptor_get_counters(raptor_ctx *ctx, uint64_t *total_steps, uint64_t *sampled_steps, uint64_t *rays);

@@ -24,7 +24,7 @@ STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 
 SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_render_disk",
            "raptor_line_profile", "raptor_set_camera_time", "raptor_set_window", "raptor_upload_snapshot",
            "raptor_light_curve", "raptor_spectrum", "raptor_flux",
-           "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_get_counters", "raptor_fp64_peak",
+           "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_null_norm", "raptor_get_counters", "raptor_fp64_peak",
            "raptor_destroy", "raptor_last_error")
 
 
@@ -81,6 +81,7 @@ def lib():
         L.raptor_render_host.argtypes = [vp, vp, vp, vp, vp]
         L.raptor_trace.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
         L.raptor_eval_rhs.argtypes = [vp, i32, vp, vp, vp]
+        L.raptor_null_norm.argtypes = [vp, i32, vp, vp, vp]
         L.raptor_get_counters.argtypes = [vp, u64p, u64p, u64p]
         L.raptor_fp64_peak.argtypes = [i32, dp, dp]
         L.raptor_destroy.argtypes = [vp]
@@ -190,6 +191,10 @@ def raptor_trace(ctx, n, d_alpha, d_beta, d_I=None, d_tau=None, d_XK=None, d_sta
 
 def raptor_eval_rhs(ctx, n, d_XK, d_f, stream=None):
     _check(lib().raptor_eval_rhs(ctx, n, d_XK, d_f, stream), ctx)
+
+
+def raptor_null_norm(ctx, n, d_XK, d_out, stream=None):
+    _check(lib().raptor_null_norm(ctx, n, d_XK, d_out, stream), ctx)
 
 
 def raptor_get_counters(ctx):
@@ -334,6 +339,15 @@ class Raptor:
         raptor_eval_rhs(self.ctx, q.shape[0], q.data_ptr(), f.data_ptr(), _stream_ptr())
         torch.cuda.synchronize()
         return f.cpu().numpy()
+
+    def null_norm(self, XK):
+        """g_mn k^m k^n (Eq. 4) at the states XK[n][8]."""
+        import torch
+        q = torch.as_tensor(np.ascontiguousarray(XK, dtype=np.float64)).cuda()
+        out = torch.empty((q.shape[0],), dtype=torch.float64, device="cuda")
+        raptor_null_norm(self.ctx, q.shape[0], q.data_ptr(), out.data_ptr(), _stream_ptr())
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
 
     def counters(self):
         return raptor_get_counters(self.ctx)

@@ -156,6 +156,27 @@ __global__ void k_eval_rhs(const __grid_constant__ KP P, int n, const double* __
     f[i * 4 + 0] = f0; f[i * 4 + 1] = f1; f[i * 4 + 2] = f2; f[i * 4 + 3] = f3;
 }
 
+// diagnostics: null condition g_mn k^m k^n (Eq. 4) at given states
+template <bool H1>
+__global__ void k_null_norm(const __grid_constant__ KP P, int n, const double* __restrict__ XK, double* __restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double* q = XK + (size_t)i * 8;
+    Geom G;
+    geom_eval<H1>(P, q[1], q[2], G);
+    Met M;
+    met_eval(P, G, M);
+    const double kt = q[4], kr = G.ex * q[5], kh = G.dth * q[6], kp = q[7];
+    out[i] = ks_dot(M, kt, kr, kh, kp, kt, kr, kh, kp);
+}
+
+cudaError_t launch_null_norm(const KP& P, int n, const double* d_XK, double* d_out, cudaStream_t stream) {
+    int grid = (n + 127) / 128;
+    if (P.omh == 0.0) k_null_norm<true><<<grid, 128, 0, stream>>>(P, n, d_XK, d_out);
+    else k_null_norm<false><<<grid, 128, 0, stream>>>(P, n, d_XK, d_out);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_eval_rhs(const KP& P, int n, const double* d_XK, double* d_f, cudaStream_t stream) {
     int grid = (n + 127) / 128;
     if (P.omh == 0.0) k_eval_rhs<true><<<grid, 128, 0, stream>>>(P, n, d_XK, d_f);

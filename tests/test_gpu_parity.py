@@ -438,3 +438,25 @@ def test_radial_offset_negative_spin_and_rectangular_pixels(rb, orc, cfg):
     else:
         s = replace(scenes.config_C2(nx=36), ny=20, mks_r0=0.4, r_cam=250.0, incl_deg=140.0)
     check_full(rb, orc, s)
+
+
+def test_null_condition_along_gpu_rays(rb, orc):
+    # Eq. 4: the camera wavevector is null to round-off and stays null to truncation along GPU rays;
+    # the diagnostic kernel agrees with the oracle's metric contraction at the same states
+    s = scenes.Scene(a=0.9375, mks_h=0.3, incl_deg=60.0)
+    o = orc.Oracle(s)
+    rng = np.random.default_rng(4)
+    al, be = rng.uniform(-18, 18, 32), rng.uniform(-18, 18, 32)
+    cam = np.array([np.concatenate(o.camera(x, y)) for x, y in zip(al, be)])
+    with rb.Raptor(s) as R:
+        g = R.trace(al, be)
+        n_cam = R.null_norm(cam)
+        n_end = R.null_norm(g["XK"])
+    kt2_cam, kt2_end = cam[:, 4] ** 2, g["XK"][:, 4] ** 2
+    assert np.abs(n_cam / kt2_cam).max() < 1e-12
+    esc = g["status"] == 2
+    rel = np.abs(n_end[esc] / kt2_end[esc])                                          # policy-A truncation (P4)
+    assert esc.sum() > 10 and rel.max() < 2e-3 and np.median(rel) < 2e-5
+    for i in range(0, 32, 4):
+        ref = o.null_norm(g["XK"][i, :4], g["XK"][i, 4:])
+        assert abs(n_end[i] - ref) <= 1e-9 * kt2_end[i] + 1e-12 * abs(ref)
