@@ -391,3 +391,33 @@ def test_flux_is_the_pixel_sum_in_jansky():
     L = 6.6743e-8 * s.M_bh_g / C_ ** 2
     expect = img.sum() * (s.fov_M / 4) ** 2 * L ** 2 / s.D_src_cm ** 2 * 1e23
     assert o.flux(img)[0] == pytest.approx(expect, rel=1e-13)
+
+
+# ------------------------------------------------------------------------------------ P14
+def _c1_flux(nx, refine=1.0):
+    s = scenes.config_C1(nx)
+    s = replace(s, step_c=s.step_c / refine, step_min=s.step_min / refine, step_max=s.step_max / refine,
+                eps_polar=s.eps_polar / refine)
+    o = orc.Oracle(s)
+    out = o.render()
+    return o.flux(out["image"])[0], out
+
+
+def test_P14_whole_image_step_refinement_and_resolution_convergence():
+    # (i) the geodesics are 4th order, the quadrature of Eq. 37 with one end-point sample per step [A8] is 1st
+    # order: halving every step halves the flux error.  (iii) the total flux converges with the image resolution,
+    # the differences between successive resolutions shrinking as in Table 3.
+    f1, _ = _c1_flux(24, 1.0)
+    f2, _ = _c1_flux(24, 2.0)
+    f4, _ = _c1_flux(24, 4.0)
+    assert abs(f1 - f2) / f4 < 0.05                       # the contract step rule is within a few % of converged
+    assert 1.5 < (f1 - f2) / (f2 - f4) < 2.7, ((f1 - f2) / (f2 - f4))
+    fr = [_c1_flux(n)[0] for n in (8, 16, 32, 64)]
+    d = np.abs(np.diff(fr))
+    assert d[2] < d[0] and d[2] / fr[-1] < 0.05, (fr, d)
+    # every pixel's intensity is non-negative and the image is mirror-symmetric about beta = 0 only in flux
+    # between the two halves for the equatorially symmetric torus seen from i = 60 deg: NOT symmetric (Doppler
+    # boosting): the approaching side (alpha < 0, Eq. 25) is brighter
+    _, out = _c1_flux(32)
+    img = out["image"][0]
+    assert (img >= 0).all() and img[:, :16].sum() > 1.2 * img[:, 16:].sum()
