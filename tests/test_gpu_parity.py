@@ -460,3 +460,20 @@ def test_null_condition_along_gpu_rays(rb, orc):
     for i in range(0, 32, 4):
         ref = o.null_norm(g["XK"][i, :4], g["XK"][i, 4:])
         assert abs(n_end[i] - ref) <= 1e-9 * kt2_end[i] + 1e-12 * abs(ref)
+
+
+# ------------------------------------------------- full sizes, whole rows: the launch configuration bench.py times
+@pytest.mark.parametrize("cfg", ["C1", "C2", "C4"])
+def test_full_size_rows_against_the_oracle(rb, orc, cfg):
+    s = scenes.config(cfg)
+    g = gpu_render(rb, s)
+    stride = s.ny // 8
+    ref = orc.Oracle(s).render(rows=(stride // 2, s.ny), row_stride=stride)        # 8 full rows of the image
+    rows = np.arange(stride // 2, s.ny, stride)
+    keep = ~ring_mask(s)[rows]
+    err = rel_err(g["image"][:, rows], ref["image"][:, rows])[0]
+    assert (g["status"][rows][keep] == ref["status"][rows][keep]).all()
+    assert (g["nsteps"][rows][keep] == ref["nsteps"][rows][keep]).mean() >= 0.999
+    assert (err[keep] <= 1e-8).mean() >= 0.999, (cfg, np.sort(err[keep])[-5:])
+    fo, fg = ref["image"][0, rows].sum(), g["image"][0, rows].sum()
+    assert abs(fg - fo) <= 1e-9 * abs(fo)                                          # flux of these rows
