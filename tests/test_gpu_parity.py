@@ -477,3 +477,12 @@ def test_full_size_rows_against_the_oracle(rb, orc, cfg):
     assert (err[keep] <= 1e-8).mean() >= 0.999, (cfg, np.sort(err[keep])[-5:])
     fo, fg = ref["image"][0, rows].sum(), g["image"][0, rows].sum()
     assert abs(fg - fo) <= 1e-9 * abs(fo)                                          # flux of these rows
+
+
+@pytest.mark.parametrize("n_freq", [2, 3, 33, 64])
+def test_frequency_counts_even_odd_and_maximum(rb, orc, n_freq):
+    # 64 = RAPTOR_MAX_FREQ: 224 KB of shared memory per CTA (1 x 7 warps); odd counts exercise the tail of the
+    # two-at-a-time transfer loop
+    s = scenes.config_C3(nx=16, n_freq=n_freq)
+    g, ref, rep = check_full(rb, orc, s)
+    assert g["image"].shape[0] == n_freq
