@@ -486,3 +486,33 @@ def test_frequency_counts_even_odd_and_maximum(rb, orc, n_freq):
     s = scenes.config_C3(nx=16, n_freq=n_freq)
     g, ref, rep = check_full(rb, orc, s)
     assert g["image"].shape[0] == n_freq
+
+
+# ------------------------------------------------- tile sharding of one image (8(e)) and empty inputs
+def test_tile_shards_sum_to_the_full_image_and_empty_shards_write_nothing(rb):
+    from paper_1801_10452_b200 import parallel
+    s = replace(scenes.config_C2(nx=44), ny=26)
+    with rb.Raptor(s) as R:
+        full, status, nsteps = R.render()
+        world = 3
+        acc = torch.zeros_like(full)
+        owner = parallel.pixel_owner_map(s.nx, s.ny, world).cuda()
+        for r in range(world):
+            R.set_shard(r, world)
+            part = torch.zeros_like(full)
+            R.render(want_status=False, image=part)
+            assert bool((part[0][owner != r] == 0).all())          # touches only its own tiles
+            acc += part
+        assert torch.equal(acc, full)                              # disjoint support: exact
+        # more ranks than tiles: the surplus ranks trace nothing and leave the buffer untouched
+        ntiles = parallel.n_tiles(s.nx, s.ny)
+        R.set_shard(ntiles + 2, ntiles + 5)
+        untouched = torch.full_like(full, -7.0)
+        R.render(want_status=False, image=untouched)
+        torch.cuda.synchronize()
+        assert bool((untouched == -7.0).all())
+        R.set_shard(0, 1)
+        # empty ray list
+        rb.raptor_trace(R.ctx, 0, None, None)
+        before = R.counters()
+        assert R.counters() == before
