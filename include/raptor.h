@@ -171,8 +171,9 @@ int raptor_trace(raptor_ctx *ctx, int32_t n, const double *d_alpha, const double
 int raptor_eval_rhs(raptor_ctx *ctx, int32_t n, const double *d_XK, double *d_f, void *cuda_stream);
 
 /* Diagnostics: the null condition g_mn k^m k^n (Eq. 4) at n states, d_XK[n][8] in (e.g. the final
- * states raptor_trace returns), d_out[n] out (device).  0 up to the integrator's truncation error. */
-int raptor_null_norm(raptor_ctx *ctx, int32_t n, const double *d_XK, double *d_out, void *cuda_stream);
+ * states raptor_trace returns), d_out[n] out (device): 0 up to the integrator's truncation error.  d_ELQ_or_null
+ * (device, [n][3]) receives the constants of motion E = -k_t, L = k_phi, Q of Eq. 38-40. */
+int raptor_null_norm(raptor_ctx *ctx, int32_t n, const double *d_XK, double *d_out, double *d_ELQ_or_null, void *cuda_stream);
 
 /* Counters accumulated by every render / trace since creation (synchronises the context's work):
  * accepted RK4 steps, steps on which plasma was sampled, rays traced. */

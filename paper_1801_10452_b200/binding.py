@@ -81,7 +81,7 @@ def lib():
         L.raptor_render_host.argtypes = [vp, vp, vp, vp, vp]
         L.raptor_trace.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
         L.raptor_eval_rhs.argtypes = [vp, i32, vp, vp, vp]
-        L.raptor_null_norm.argtypes = [vp, i32, vp, vp, vp]
+        L.raptor_null_norm.argtypes = [vp, i32, vp, vp, vp, vp]
         L.raptor_get_counters.argtypes = [vp, u64p, u64p, u64p]
         L.raptor_fp64_peak.argtypes = [i32, dp, dp]
         L.raptor_destroy.argtypes = [vp]
@@ -193,8 +193,8 @@ def raptor_eval_rhs(ctx, n, d_XK, d_f, stream=None):
     _check(lib().raptor_eval_rhs(ctx, n, d_XK, d_f, stream), ctx)
 
 
-def raptor_null_norm(ctx, n, d_XK, d_out, stream=None):
-    _check(lib().raptor_null_norm(ctx, n, d_XK, d_out, stream), ctx)
+def raptor_null_norm(ctx, n, d_XK, d_out, d_ELQ=None, stream=None):
+    _check(lib().raptor_null_norm(ctx, n, d_XK, d_out, d_ELQ, stream), ctx)
 
 
 def raptor_get_counters(ctx):
@@ -340,14 +340,16 @@ class Raptor:
         torch.cuda.synchronize()
         return f.cpu().numpy()
 
-    def null_norm(self, XK):
-        """g_mn k^m k^n (Eq. 4) at the states XK[n][8]."""
+    def null_norm(self, XK, with_constants=False):
+        """g_mn k^m k^n (Eq. 4) at the states XK[n][8]; with_constants: also (E, L, Q) of Eq. 38-40, [n][3]."""
         import torch
         q = torch.as_tensor(np.ascontiguousarray(XK, dtype=np.float64)).cuda()
         out = torch.empty((q.shape[0],), dtype=torch.float64, device="cuda")
-        raptor_null_norm(self.ctx, q.shape[0], q.data_ptr(), out.data_ptr(), _stream_ptr())
+        elq = torch.empty((q.shape[0], 3), dtype=torch.float64, device="cuda") if with_constants else None
+        raptor_null_norm(self.ctx, q.shape[0], q.data_ptr(), out.data_ptr(), elq.data_ptr() if with_constants else None,
+                         _stream_ptr())
         torch.cuda.synchronize()
-        return out.cpu().numpy()
+        return (out.cpu().numpy(), elq.cpu().numpy()) if with_constants else out.cpu().numpy()
 
     def counters(self):
         return raptor_get_counters(self.ctx)

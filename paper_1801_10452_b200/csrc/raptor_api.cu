@@ -466,11 +466,11 @@ extern "C" int raptor_eval_rhs(raptor_ctx* ctx, int32_t n, const double* d_XK, d
     return RAPTOR_OK;
 }
 
-extern "C" int raptor_null_norm(raptor_ctx* ctx, int32_t n, const double* d_XK, double* d_out, void* cuda_stream) {
+extern "C" int raptor_null_norm(raptor_ctx* ctx, int32_t n, const double* d_XK, double* d_out, double* d_ELQ_or_null, void* cuda_stream) {
     if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
     if (n < 0 || (n > 0 && (!d_XK || !d_out))) return fail(ctx, RAPTOR_EINVAL, "n < 0 or NULL buffer");
     if (n == 0) return RAPTOR_OK;
-    CK(ctx, launch_null_norm(ctx->kp, n, d_XK, d_out, (cudaStream_t)cuda_stream));
+    CK(ctx, launch_null_norm(ctx->kp, n, d_XK, d_out, d_ELQ_or_null, (cudaStream_t)cuda_stream));
     return RAPTOR_OK;
 }
 

@@ -158,7 +158,8 @@ __global__ void k_eval_rhs(const __grid_constant__ KP P, int n, const double* __
 
 // diagnostics: null condition g_mn k^m k^n (Eq. 4) at given states
 template <bool H1>
-__global__ void k_null_norm(const __grid_constant__ KP P, int n, const double* __restrict__ XK, double* __restrict__ out) {
+__global__ void k_null_norm(const __grid_constant__ KP P, int n, const double* __restrict__ XK, double* __restrict__ out,
+                            double* __restrict__ elq) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const double* q = XK + (size_t)i * 8;
@@ -168,12 +169,21 @@ __global__ void k_null_norm(const __grid_constant__ KP P, int n, const double* _
     met_eval(P, G, M);
     const double kt = q[4], kr = G.ex * q[5], kh = G.dth * q[6], kp = q[7];
     out[i] = ks_dot(M, kt, kr, kh, kp, kt, kr, kh, kp);
+    if (elq) {
+        // Eq. 38-40: E = -k_t, L = k_phi, Q = k_th^2 + cos^2 th (-a^2 k_t^2 + k_phi^2 / sin^2 th)
+        const double k_t = ks_dot(M, kt, kr, kh, kp, 1.0, 0.0, 0.0, 0.0);               // g(k, d_t)
+        const double k_p = ks_dot(M, kt, kr, kh, kp, 0.0, 0.0, 0.0, 1.0);               // g(k, d_phi)
+        const double k_h = M.Sig * kh;
+        elq[i * 3 + 0] = -k_t;
+        elq[i * 3 + 1] = k_p;
+        elq[i * 3 + 2] = fma(k_h, k_h, G.c * G.c * (k_p * k_p / M.ss - P.a2 * k_t * k_t));
+    }
 }
 
-cudaError_t launch_null_norm(const KP& P, int n, const double* d_XK, double* d_out, cudaStream_t stream) {
+cudaError_t launch_null_norm(const KP& P, int n, const double* d_XK, double* d_out, double* d_elq, cudaStream_t stream) {
     int grid = (n + 127) / 128;
-    if (P.omh == 0.0) k_null_norm<true><<<grid, 128, 0, stream>>>(P, n, d_XK, d_out);
-    else k_null_norm<false><<<grid, 128, 0, stream>>>(P, n, d_XK, d_out);
+    if (P.omh == 0.0) k_null_norm<true><<<grid, 128, 0, stream>>>(P, n, d_XK, d_out, d_elq);
+    else k_null_norm<false><<<grid, 128, 0, stream>>>(P, n, d_XK, d_out, d_elq);
     return cudaGetLastError();
 }
 

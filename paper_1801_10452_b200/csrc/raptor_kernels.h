@@ -47,7 +47,7 @@ cudaError_t launch_flux(const double* d_image, size_t npix, int n_freq, double s
                         double* d_flux, cudaStream_t stream);
 cudaError_t launch_profile(const double* d_image, const double* d_red, size_t npix, int nbins, double g_min, double g_max,
                            double scale, double* d_partial, double* d_hist, cudaStream_t stream);
-cudaError_t launch_null_norm(const KP& P, int n, const double* d_XK, double* d_out, cudaStream_t stream);
+cudaError_t launch_null_norm(const KP& P, int n, const double* d_XK, double* d_out, double* d_elq, cudaStream_t stream);
 cudaError_t launch_eval_rhs(const KP& P, int n, const double* d_XK, double* d_f, cudaStream_t stream);
 cudaError_t launch_fp64_peak(int iters, int blocks, double* d_out, cudaStream_t stream);
 

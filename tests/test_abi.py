@@ -70,6 +70,7 @@ def test_validation_of_grid_and_frequencies(lib):
 def test_null_handles_are_errors_not_crashes(lib):
     assert lib.raptor_render(None, None, None, None, None) == binding.EINVAL
     assert lib.raptor_spectrum(None, None, None, None) == binding.EINVAL
+    assert lib.raptor_null_norm(None, 1, None, None, None, None) == binding.EINVAL
     assert lib.raptor_render_disk(None, None, None, None, None, None) == binding.EINVAL
     assert lib.raptor_line_profile(None, None, None, 10, 0.0, 1.0, None, None) == binding.EINVAL
     assert lib.raptor_light_curve(None, 1, 0.0, 1.0, None, None) == binding.EINVAL

@@ -460,6 +460,19 @@ def test_null_condition_along_gpu_rays(rb, orc):
     for i in range(0, 32, 4):
         ref = o.null_norm(g["XK"][i, :4], g["XK"][i, 4:])
         assert abs(n_end[i] - ref) <= 1e-9 * kt2_end[i] + 1e-12 * abs(ref)
+    # constants of motion (Eq. 38-40): the camera gives E = 1, L = -alpha sin i, Q of Eq. 26; they drift by the
+    # truncation error only, and the kernel agrees with the oracle's evaluation at the same states
+    with rb.Raptor(s) as R:
+        _, c_cam = R.null_norm(cam, with_constants=True)
+        _, c_end = R.null_norm(g["XK"], with_constants=True)
+    si, ci = math.sin(math.radians(60.0)), math.cos(math.radians(60.0))
+    assert np.abs(c_cam[:, 0] - 1.0).max() < 1e-12 and np.abs(c_cam[:, 1] + al * si).max() < 1e-11
+    assert np.abs(c_cam[:, 2] - (be ** 2 + ci ** 2 * (al ** 2 - s.a ** 2))).max() < 1e-9
+    drift = np.abs(c_end[esc] - c_cam[esc])
+    assert np.median(drift[:, 0]) < 1e-5 and np.median(drift[:, 1]) < 1e-4
+    for i in range(0, 32, 4):
+        E, L, Q = o.conserved(g["XK"][i, :4], g["XK"][i, 4:])
+        assert np.allclose(c_end[i], [E, L, Q], rtol=1e-9, atol=1e-9)
 
 
 # ------------------------------------------------- full sizes, whole rows: the launch configuration bench.py times
