@@ -26,10 +26,13 @@
  * Bardeen critical curve incl. Table 1 of the paper, flat-space straight lines, redshift
  * closed forms, uniform-slab closed forms (I = jL, I = S(1-exp(-tau)), I -> B_nu), the
  * emissivity fit against direct quadrature over the Maxwell-Juettner distribution, the
- * cyclotron frequency the paper prints, multilinear-interpolation exactness.
- * Parity unpinned (definitions, not derivable -- see DESIGN.md): the step-rule constants of
- * BASELINE.json configs[0], the end-point sampling of the quadrature [A8], the amplitudes of
- * the synthetic plasma models, and Table 3 / Fig. 7-13 of the paper (datasets absent).
+ * cyclotron frequency the paper prints, multilinear-interpolation exactness,
+ * both step rules (Eq. 21-24 and the configs[0] clamp with and without the polar guard), the
+ * optical-depth cut-off exit, pixel centres and the [k][iy][ix] image layout by hand computation.
+ * Parity unpinned (definitions, not derivable -- see DESIGN.md): the VALUES of the step-rule
+ * constants of BASELINE.json configs[0] and of eps_polar, the end-point sampling of the quadrature
+ * [A8], the amplitudes of the synthetic plasma models, and Table 3 / Fig. 7-13 of the paper
+ * (datasets absent).  Every function of this file has a pin.
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/oracle.py does it).
  */

@@ -374,3 +374,94 @@ def test_P13_redshift_of_a_free_falling_emitter_on_a_radial_ray():
         nu_hat = -(K @ g @ pl["u"])
         # K carries the truncation error of the policy-A steps, amplified ~1/(r - 2) near the horizon
         assert nu_hat == pytest.approx(1.0 / (1.0 - math.sqrt(2.0 / r)), rel=2e-7 if r > 3.0 else 5e-6)
+
+
+# ------------------------------------------------------------------------- step rules, pixel grid, layout
+# Hand-computed expectations: none of the numbers below comes from orc_step_size / orc_pixel_ab themselves.
+def test_step_policy_B_is_eq21_to_24_by_hand():
+    # Eq. 21-24: dl_1 = eps/(|K^1|+delta), dl_2 = eps min(x2, 1-x2)/(|K^2|+delta),
+    # dl_3 = eps/(|K^phi|+delta), dl = 1/(1/dl_1 + 1/dl_2 + 1/dl_3).  delta = 1e-40 is invisible in double.
+    o = orc.Oracle(vac(a=0.9375, h=0.3, step_policy=1, eps=0.03, delta=1e-40))
+    K = [7.7, 0.5, -0.25, 0.1]                               # K^t must not enter
+    # x2 = 0.2: 1/dl = (0.5 + 0.25/0.2 + 0.1)/0.03
+    assert o.step_size([0.0, 2.0, 0.2, 1.0], K) == pytest.approx(0.03 / (0.5 + 1.25 + 0.1), rel=1e-14)
+    # x2 = 0.7: min(x2, 1 - x2) = 0.3 (dropping the min gives 0.03/(0.5 + 0.25/0.7 + 0.1): different by 34 %)
+    assert o.step_size([0.0, 2.0, 0.7, 1.0], K) == pytest.approx(0.03 / (0.5 + 0.25 / 0.3 + 0.1), rel=1e-14)
+    # beyond the pole the coordinate is folded back into [0, 1]: x2 = 1.3 -> 0.7, x2 = -0.2 -> 0.2
+    assert o.step_size([0.0, 2.0, 1.3, 1.0], K) == pytest.approx(0.03 / (0.5 + 0.25 / 0.3 + 0.1), rel=1e-13)
+    assert o.step_size([0.0, 2.0, -0.2, 1.0], K) == pytest.approx(0.03 / (0.5 + 1.25 + 0.1), rel=1e-13)
+    # harmonic, not arithmetic, sum: one dominant component sets the step; signs do not matter; linear in eps
+    assert o.step_size([0.0, 2.0, 0.5, 1.0], [1.0, -3.0, 0.0, 0.0]) == pytest.approx(0.03 / 3.0, rel=1e-13)
+    assert o.step_size([0.0, 2.0, 0.5, 1.0], [1.0, 0.0, 0.0, -2.0]) == pytest.approx(0.03 / 2.0, rel=1e-13)
+    o2 = orc.Oracle(vac(a=0.9375, h=0.3, step_policy=1, eps=0.06, delta=1e-40))
+    assert o2.step_size([0.0, 2.0, 0.2, 1.0], K) == pytest.approx(0.06 / 1.85, rel=1e-14)
+    # delta regularises a vanishing wavevector: K = 0 gives 1/(3 delta/eps + 2 delta/eps...) finite and huge
+    o3 = orc.Oracle(vac(a=0.0, h=1.0, step_policy=1, eps=0.03, delta=1e-3))
+    assert o3.step_size([0.0, 2.0, 0.25, 0.0], [1.0, 0.0, 0.0, 0.0]) == pytest.approx(0.03 / (1e-3 + 1e-3 / 0.25 + 1e-3), rel=1e-13)
+
+
+def test_step_policy_A_clamp_and_polar_guard_by_hand():
+    # BASELINE.json configs[0]: h = 0.05 (r - r_H) clamped to [1e-3, 1]; [A6] adds h <= eps_polar r |sin theta|
+    # floored at 1e-3.  theta = pi x2 for h = 1.
+    a = 0.9375
+    rH = 1.0 + math.sqrt(1.0 - a * a)
+    o = orc.Oracle(vac(a=a, h=1.0))                          # eps_polar = 0.125 (default)
+    K = [1.0, 0.1, 0.1, 0.1]                                 # policy A does not look at K
+    eq = 0.5                                                 # x2 = 1/2: the equator, guard inactive
+    assert o.step_size([0, math.log(1000.0), eq, 0], K) == 1.0                                    # upper clamp
+    assert o.step_size([0, math.log(21.0 + rH), eq, 0], K) == pytest.approx(1.0, rel=1e-12)       # 0.05 * 21 > 1
+    assert o.step_size([0, math.log(3.0), eq, 0], K) == pytest.approx(0.05 * (3.0 - rH), rel=1e-13)
+    assert o.step_size([0, math.log(1.4), eq, 0], K) == pytest.approx(0.05 * (1.4 - rH), rel=1e-12)
+    assert o.step_size([0, math.log(rH + 0.01), eq, 0], K) == 1e-3                                # lower clamp
+    # the horizon radius enters: Schwarzschild r_H = 2
+    o0 = orc.Oracle(vac(a=0.0, h=1.0))
+    assert o0.step_size([0, math.log(6.0), eq, 0], K) == pytest.approx(0.05 * 4.0, rel=1e-13)
+    # polar guard at theta = 0.01 rad: on -> 0.125 r sin(0.01); off (eps_polar = 1e30) -> the radial rule alone
+    x2 = 0.01 / math.pi
+    for r in (1000.0, 8.0):
+        radial = min(max(0.05 * (r - rH), 1e-3), 1.0)
+        assert o.step_size([0, math.log(r), x2, 0], K) == pytest.approx(min(radial, 0.125 * r * math.sin(0.01)), rel=1e-12)
+        assert o.step_size([0, math.log(r), 1.0 - x2, 0], K) == pytest.approx(min(radial, 0.125 * r * math.sin(0.01)), rel=1e-9)
+    off = orc.Oracle(vac(a=a, h=1.0, eps_polar=1e30))
+    assert off.step_size([0, math.log(8.0), x2, 0], K) == pytest.approx(0.05 * (8.0 - rH), rel=1e-13)
+    # the guard is floored at step_min as well, and uses |sin|: beyond the pole (x2 < 0) it is still positive
+    assert o.step_size([0, math.log(3.0), 1e-6, 0], K) == 1e-3
+    assert o.step_size([0, math.log(8.0), -x2, 0], K) == pytest.approx(0.125 * 8.0 * math.sin(0.01), rel=1e-9)
+    # other constants of the rule are parameters
+    o5 = orc.Oracle(vac(a=a, h=1.0, step_c=0.02, step_min=0.01, step_max=0.25))
+    assert o5.step_size([0, math.log(5.0), eq, 0], K) == pytest.approx(0.02 * (5.0 - rH), rel=1e-13)
+    assert o5.step_size([0, math.log(500.0), eq, 0], K) == 0.25 and o5.step_size([0, math.log(1.4), eq, 0], K) == 0.01
+
+
+def test_pixel_centres_and_image_layout_by_hand():
+    # [A4b]: alpha_ix = (ix + 1/2) fov/nx - fov/2, beta_iy likewise; image[k][iy][ix], status/nsteps [iy][ix].
+    s = replace(scenes.config_C3(nx=5, n_freq=2, n1=32, n2=32), ny=3, fov_M=30.0)
+    o = orc.Oracle(s)
+    assert o.pixel_ab(0, 0) == pytest.approx((-15.0 + 3.0, -15.0 + 5.0), abs=1e-14)      # fov/(2 nx) = 3, fov/(2 ny) = 5
+    assert o.pixel_ab(4, 2) == pytest.approx((15.0 - 3.0, 15.0 - 5.0), abs=1e-14)
+    assert o.pixel_ab(2, 1) == pytest.approx((0.0, 0.0), abs=1e-14)
+    assert o.pixel_ab(1, 0)[0] - o.pixel_ab(0, 0)[0] == pytest.approx(6.0, abs=1e-14)    # ix <-> alpha
+    assert o.pixel_ab(0, 1)[1] - o.pixel_ab(0, 0)[1] == pytest.approx(10.0, abs=1e-14)   # iy <-> beta
+    # a 6 x 4 render of an asymmetric scene (Kerr, i = 20 deg, seeded grid): every pixel equals the single ray
+    # traced at the hand-computed impact parameters -- a transposed image, a missing +1/2 or swapped frequency
+    # planes would all fail
+    s = replace(scenes.config_C3(nx=6, n_freq=2, n1=32, n2=32), ny=4, fov_M=24.0)
+    o = orc.Oracle(s)
+    out = o.render()
+    assert out["image"].shape == (2, 4, 6) and out["status"].shape == (4, 6)
+    seen = set()
+    for iy in range(4):
+        for ix in range(6):
+            al, be = (ix + 0.5) * 24.0 / 6 - 12.0, (iy + 0.5) * 24.0 / 4 - 12.0
+            r = o.trace(al, be)
+            assert np.array_equal(out["image"][:, iy, ix], r["I"]), (ix, iy)
+            assert out["status"][iy, ix] == r["status"] and out["nsteps"][iy, ix] == r["nsteps"]
+            seen.add(float(r["I"][0]))
+    assert len(seen) == 24                                   # no two pixels alike: the comparison discriminates
+    assert out["steps"] == int(out["nsteps"].sum())
+    # orientation by physics: the approaching side of the prograde flow is alpha < 0 (L = -alpha sin i > 0, Eq. 25),
+    # i.e. the LEFT half of every row, and it is Doppler-brighter
+    c1 = orc.Oracle(replace(scenes.config_C1(8), ny=4)).render()["image"][0]
+    assert c1.shape == (4, 8) and c1[:, :4].sum() > 1.2 * c1[:, 4:].sum()
+    b = np.unravel_index(np.argmax(c1), c1.shape)
+    assert b[1] < 4 and b[0] in (1, 2)                       # brightest pixel: left half, one of the two central rows
