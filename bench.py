@@ -30,21 +30,14 @@ if ROOT not in sys.path:
 METRIC = "geodesic_steps_per_sec"
 UNIT = "steps/s"
 
-# FP64 peak of one B200 for "bound": "alu": 148 SMs x 4 sub-partitions x 16 FP64 FMA
-# lanes x 2 flop x 1.965 GHz (clocks.max.sm).  The live DFMA probe (raptor_fp64_peak) is reported beside it.
-FP64_PEAK_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
-
-# FP64 work per accepted integrator step of each workload: thread-level executed
-# (DFMA, DMUL, DADD) of the shipped k_render kernel divided by the accepted steps, counted with ncu
-# (profiles/flop_per_step_r1.md).  flop = 2 DFMA + DMUL + DADD.  It contains the RHS evaluations with their
-# exp / sin / cos, the integrator's combination and the sampled steps' share of sampler + transfer arithmetic.
-# Integer and control instructions are not counted.  C3's figure is for its 32 frequencies.
-FP64_INST_PER_STEP = {"C0": (476.5, 335.9, 101.1), "C1": (200.2, 225.1, 20.2), "C2": (235.5, 255.6, 24.7),
-                      "C3": (369.4, 293.3, 39.3), "C4": (245.1, 257.1, 30.7), "PB1": (261.8, 171.9, 32.1),
-                      "LC": (257.0, 260.4, 31.9)}
-FLOP_PER_STEP = {k: 2.0 * v[0] + v[1] + v[2] for k, v in FP64_INST_PER_STEP.items()}
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_render launch (ncu --set full, profiles/k_render_C2_r1.md)
-DRAM_BYTES_PER_LAUNCH = {"C2": 4.264e6 + 0.035e6}
+# FP64 peak of one B200 for "bound": "alu".  The denominator of roofline.frac is the MEASURED
+# peak: the live DFMA probe raptor_fp64_peak (8 independent DFMA chains per thread on all SMs), run in this process
+# right before the timed region.  The derived figure 148 SMs x 4 sub-partitions x 16 FP64 FMA lanes x 2 flop x
+# 1.965 GHz (clocks.max.sm) is printed beside it as peak_nominal.
+FP64_PEAK_NOMINAL_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
+# The numerator: executed FP64 instructions per accepted step of the SHIPPED kernel, measured by ncu and stored in
+# profiles/fp64_inst_per_step.json together with the hash of the kernel sources (paper_1801_10452_b200/
+# roofline_counts.py says how).  If the sources here hash differently the roofline is reported as null.
 # paper's own numbers for its performance configuration (Table B.1 / PAPER.md:342, 666): context for PB1 only
 PAPER_GEODESICS_PER_SEC = {"GTX 1080, OpenACC, single precision": 104900.0, "i7-6950X 10 cores, OpenMP, single precision": 10707.0}
 
@@ -60,10 +53,6 @@ def build_scene(workload: str):
         s = scenes.config_C4(nx=256, n1=64, n2=48, n3=32, nt=16)
         return replace(s, name="LC", freq_hz=(22e9, 43e9, 86e9, 230e9))
     return scenes.config(workload)
-
-
-def algorithmic_flops(scene, workload, steps, sampled):
-    return steps * FLOP_PER_STEP[workload]
 
 
 # ------------------------------------------------------------------------------------------------
@@ -140,7 +129,10 @@ def run_reference(args):
     if rank != 0:
         return
     scene = build_scene(args.workload)
-    stride = args.ref_row_stride or max(1, scene.ny // 8)     # 8 rows of the image per step
+    # rows are the oracle's only parallel axis (OpenMP, schedule(dynamic, 1)): at least 2 rows per thread per step,
+    # otherwise half the cores idle and the two oracle timings of one box (this arm, cpu_baseline) disagree
+    rows_per_step = min(scene.ny, max(8, 2 * omp_threads()))
+    stride = args.ref_row_stride or max(1, scene.ny // rows_per_step)
     for _ in range(args.warmup):
         oracle_sample(scene, max(stride, scene.ny // 2))
     tot_steps, tot_t = 0, 0.0
@@ -149,7 +141,8 @@ def run_reference(args):
         tot_steps += s
         tot_t += dt
     value = tot_steps / tot_t
-    sample = f"every {stride}th row of the {scene.nx}x{scene.ny} {args.workload} image per step ({scene.ny // stride} rows)"
+    sample = (f"every {stride}th row of the {scene.nx}x{scene.ny} {args.workload} image per step "
+              f"({len(range(stride // 2, scene.ny, stride))} rows on {omp_threads()} threads)")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -167,7 +160,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
 
-    from paper_1801_10452_b200 import binding
+    from paper_1801_10452_b200 import binding, parallel, roofline_counts
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -179,9 +172,17 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     binding.lib()
 
-    scene = build_scene(args.workload)
+    lc = args.workload == "LC"
+    strong = args.scaling == "strong" and world > 1
+    if strong and lc:
+        raise SystemExit("--scaling strong shards one image by tiles; a light curve shards by frames")
+    base_scene = build_scene(args.workload)
+    # weak scaling (default): a movie, every rank renders its OWN frame (own camera time / own snapshot);
+    # strong scaling: ONE image, every rank traces its interleaved tiles, one all-reduce(SUM) of the image per step
+    scene = base_scene if strong else parallel.frame_of_rank(base_scene, rank)
     R = binding.Raptor(scene)
-    npix = scene.nx * scene.ny
+    if strong:
+        R.set_shard(rank, world)
     image = torch.empty((scene.n_freq, scene.ny, scene.nx), dtype=torch.float64, device="cuda")
     flux = torch.empty((scene.n_freq,), dtype=torch.float64, device="cuda")
     stream = torch.cuda.current_stream()
@@ -193,34 +194,44 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    lc = args.workload == "LC"
     lc_flux = torch.empty((LC_FRAMES, scene.n_freq), dtype=torch.float64, device="cuda") if lc else None
     lc_t0 = scene.t_cam - 0.5 * LC_FRAMES * LC_DT
 
+    def render_call(img):
+        binding.raptor_render(R.ctx, img.data_ptr(), None, None, sp)
+
+    def flux_call(img):
+        binding.raptor_flux(R.ctx, img.data_ptr(), flux.data_ptr(), sp)
+        return flux
+
     def one_step(ev=None):
         # a1-a6 + image write (render kernel), a7 flux reduction (2 small kernels): 3 launches
+        if ev:
+            ev[0].record(stream)
         if lc:
             # one light curve: LC_FRAMES frames traced by one k_render launch + one flux reduction over all of them
-            if ev:
-                ev[0].record(stream)
             binding.raptor_light_curve(R.ctx, LC_FRAMES, lc_t0, LC_DT, lc_flux.data_ptr(), sp)
             if ev:
                 ev[1].record(stream)
-                ev[2].record(stream)
-            return
-        if ev:
-            ev[0].record(stream)
-        binding.raptor_render(R.ctx, image.data_ptr(), None, None, sp)
-        if ev:
-            ev[1].record(stream)
-        binding.raptor_flux(R.ctx, image.data_ptr(), flux.data_ptr(), sp)
+        elif strong:
+            # the function the gloo test drives: zero, render this rank's tiles, all-reduce the image, flux
+            def render_shard(img):
+                render_call(img)
+                if ev:
+                    ev[1].record(stream)
+            parallel.strong_step(render_shard, image, flux_call)
+        else:
+            render_call(image)
+            if ev:
+                ev[1].record(stream)
+            flux_call(image)
         if ev:
             ev[2].record(stream)
 
     for _ in range(max(args.warmup, 3)):
         one_step()
     torch.cuda.synchronize()
-    fp64_probe = binding.raptor_fp64_peak(1 << 16)[0] if rank == 0 else None
+    fp64_probe = binding.raptor_fp64_peak(1 << 16)[0]
     c_before = R.counters()
 
     sampler = ClockSampler(local)
@@ -250,18 +261,23 @@ def run_ours(args):
         g = np.ascontiguousarray(scene.grid, dtype=np.float32 if scene.grid_dtype == 1 else np.float64)
         h_grid = torch.from_numpy(g.reshape(-1).copy()).pin_memory()
     e2e_steps = max(2, min(args.steps, 5))
-
     h_lc = torch.empty((LC_FRAMES, scene.n_freq), dtype=torch.float64).pin_memory() if lc else None
 
     def e2e_step():
+        # the upload is asynchronous on the caller's stream; raptor_render_host orders itself after it (raptor.h)
         if h_grid is not None:
-            binding.raptor_upload_grid(R.ctx, h_grid.data_ptr(), h_grid.numel() * h_grid.element_size(), None)
+            binding.raptor_upload_grid(R.ctx, h_grid.data_ptr(), h_grid.numel() * h_grid.element_size(), sp)
         if lc:
             binding.raptor_light_curve(R.ctx, LC_FRAMES, lc_t0, LC_DT, lc_flux.data_ptr(), sp)
             h_lc.copy_(lc_flux, non_blocking=True)
             torch.cuda.synchronize()
-            return
-        binding.raptor_render_host(R.ctx, h_image.data_ptr(), None, None, h_flux.data_ptr())
+        elif strong:
+            one_step()
+            h_image.copy_(image, non_blocking=True)
+            h_flux.copy_(flux, non_blocking=True)
+            torch.cuda.synchronize()
+        else:
+            binding.raptor_render_host(R.ctx, h_image.data_ptr(), None, None, h_flux.data_ptr())
 
     e2e_step()
     barrier()
@@ -272,76 +288,85 @@ def run_ours(args):
     torch.cuda.synchronize()
     t_e2e = time.perf_counter() - t0
     c1 = R.counters()
-    e2e_units = c1[0] - c0[0]
 
-    # ---- aggregate over ranks: max time, summed units
-    agg = torch.tensor([total_ms, t_e2e * 1e3], dtype=torch.float64, device="cuda")
-    units = torch.tensor([float(steps_done), float(e2e_units)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(agg, op=dist.ReduceOp.MAX)
-        dist.all_reduce(units, op=dist.ReduceOp.SUM)
-    total_ms_max, e2e_ms_max = agg.tolist()
-    steps_all, e2e_units_all = units.tolist()
+    # ---- aggregate over ranks (the helper the world-size-2 gloo test covers): max time, summed units
+    total_ms_max, steps_all = parallel.aggregate(total_ms, float(steps_done), device="cuda")
+    e2e_ms_max, e2e_units_all = parallel.aggregate(t_e2e * 1e3, float(c1[0] - c0[0]), device="cuda")
+    render_ms_max, sampled_all = parallel.aggregate(sum(render_ms), float(sampled_done), device="cuda")
 
     if rank == 0:
+        frames = LC_FRAMES if lc else 1
+        images_per_step = frames * (1 if strong else world)
         value = steps_all / (total_ms_max * 1e-3)
-        images_per_s = world * args.steps * (LC_FRAMES if lc else 1) / (total_ms_max * 1e-3)
         avg_render_ms = sum(render_ms) / len(render_ms)
-        flops_launch = algorithmic_flops(scene, args.workload, steps_done / args.steps, sampled_done / args.steps)
-        achieved = flops_launch / (avg_render_ms * 1e-3) / 1e12
-        # the FP64 pipe issues one warp instruction per 2 cycles per sub-partition whether it is a DFMA or a DMUL/DADD:
-        # share of those issue slots the kernel's DFMA + DMUL + DADD fill, and the flop ceiling its mix allows
-        fi = FP64_INST_PER_STEP[args.workload]
-        n_inst = sum(fi) * steps_done / args.steps
-        pipe_frac = n_inst / (148 * 4 * 16 * 1.965e9 * avg_render_ms * 1e-3)
-        mix_ceiling = FLOP_PER_STEP[args.workload] / (2.0 * sum(fi))
-        # CPU baseline: the oracle on a bounded sample of the same workload (about 10-30 s of host work)
-        cpu = None
-        if world == 1 and not args.no_cpu_baseline:
-            stride = max(1, scene.ny // 8)
-            s, dt = oracle_sample(scene, stride)
-            if dt < 5.0:
-                s2, dt2 = oracle_sample(scene, max(1, stride // 4))
-                s, dt, stride = s2, dt2, max(1, stride // 4)
-            cpu = {"value": s / dt, "unit": UNIT, "cores": omp_threads(), "kind": "oracle",
-                   "sample": f"every {stride}th row of the {scene.nx}x{scene.ny} {args.workload} image "
-                             f"({s} steps in {dt:.1f} s)"}
-        h2d = int(h_grid.numel() * h_grid.element_size()) if h_grid is not None else 0
-        d2h = int(h_lc.numel() * 8) if lc else int(h_image.numel() * 8 + h_flux.numel() * 8)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
+            "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "strong" if strong else "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "pixels": [scene.nx, scene.ny], "n_freq": scene.n_freq,
                        "spin": scene.a, "incl_deg": scene.incl_deg, "plasma_model": scene.plasma_model,
                        "grid": [scene.nt, scene.n1, scene.n2, scene.n3], "l2": "flushed between timed iterations",
-                       "parallelism": f"frames x{world}" if world > 1 else "single GPU"},
-            "images_per_sec": images_per_s,
-            "steps_per_image": steps_done / args.steps, "sampled_steps_per_image": sampled_done / args.steps,
+                       "parallelism": ("single GPU" if world == 1 else
+                                       f"one image, interleaved 8x4 tiles over {world} ranks + all-reduce(SUM) of the image" if strong
+                                       else f"frames x{world}: every rank renders its own frame, no data-path collective")},
+            "images_per_sec": images_per_step * args.steps / (total_ms_max * 1e-3),
+            "steps_per_image": steps_all / (args.steps * images_per_step),
+            "sampled_steps_per_image": sampled_all / (args.steps * images_per_step),
             "clocks": clocks,
-            "e2e": {"value": e2e_units_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": d2h, "images_per_sec": world * e2e_steps * (LC_FRAMES if lc else 1) / (e2e_ms_max * 1e-3)},
+            "e2e": {"value": e2e_units_all / (e2e_ms_max * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": int(h_grid.numel() * h_grid.element_size()) if h_grid is not None else 0,
+                    "d2h_bytes_per_step": int(h_lc.numel() * 8) if lc else int(h_image.numel() * 8 + h_flux.numel() * 8),
+                    "images_per_sec": images_per_step * e2e_steps / (e2e_ms_max * 1e-3)},
             "gpu_launches": 3 * args.steps,
-            "frames_per_step": LC_FRAMES if lc else 1,
-            "rays_per_sec": world * args.steps * (LC_FRAMES if lc else 1) * scene.nx * scene.ny / (total_ms_max * 1e-3),
-            "roofline": {"bound": "alu", "kernel": "k_render", "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
-                         "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": DRAM_BYTES_PER_LAUNCH.get(args.workload),
-                         "fp64_pipe_frac": pipe_frac, "mix_ceiling": mix_ceiling,
-                         "fp64_inst_per_step": {"dfma": fi[0], "dmul": fi[1], "dadd": fi[2]},
-                         "peak_source": "derived: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md)",
-                         "fp64_probe_tflops": fp64_probe, "kernel_ms": avg_render_ms,
-                         "kernel_share_of_step": avg_render_ms / (total_ms / args.steps),
-                         "algorithmic_flop_per_launch": flops_launch},
-            "cpu_baseline": cpu,
+            "frames_per_step": frames,
+            "rays_per_sec": images_per_step * args.steps * scene.nx * scene.ny / (total_ms_max * 1e-3),
             "wall_s_timed_region": t_wall,
         }
+        # ---- roofline of the dominant kernel (rank 0's launches): measured counts / measured peak
+        counts, why = roofline_counts.load()
+        row = counts.get(args.workload) if counts else None
+        if row is None:
+            line["roofline"] = None
+            line["roofline_unavailable"] = why or f"no ncu counts for workload {args.workload} in profiles/fp64_inst_per_step.json"
+        else:
+            flop_step = 2.0 * row["dfma"] + row["dmul"] + row["dadd"]
+            steps_launch = steps_done / args.steps
+            achieved = steps_launch * flop_step / (avg_render_ms * 1e-3) / 1e12
+            # the FP64 pipe issues one warp instruction per 2 cycles per sub-partition whether it is a DFMA, a DMUL/DADD or
+            # a DSETP: share of those issue slots the kernel filled, and the flop ceiling its instruction mix allows
+            slots = 148 * 4 * (clocks["sm_mhz"] or 1965.0) * 1e6 / 2.0 * avg_render_ms * 1e-3 if clocks else None
+            pipe_frac = row["fp64_pipe_warp_inst"] * steps_launch / slots if slots and "fp64_pipe_warp_inst" in row else None
+            n_arith = row["dfma"] + row["dmul"] + row["dadd"]
+            line["roofline"] = {
+                "bound": "alu", "kernel": "k_render", "achieved": achieved, "peak": fp64_probe, "unit": "TFLOP/s",
+                "frac": achieved / fp64_probe,
+                "peak_source": "measured: raptor_fp64_peak (independent DFMA chains on all SMs) in this process",
+                "peak_nominal": FP64_PEAK_NOMINAL_TFLOPS, "frac_of_nominal": achieved / FP64_PEAK_NOMINAL_TFLOPS,
+                "traffic": (row.get("dram_read_bytes", 0.0) + row.get("dram_write_bytes", 0.0)) if "dram_read_bytes" in row else None,
+                "fp64_pipe_frac": pipe_frac, "mix_ceiling": flop_step / (2.0 * n_arith),
+                "fp64_inst_per_step": {"dfma": row["dfma"], "dmul": row["dmul"], "dadd": row["dadd"],
+                                       "pipe_warp_inst_x32": 32.0 * row.get("fp64_pipe_warp_inst", float("nan"))},
+                "counts_source": "profiles/fp64_inst_per_step.json (ncu, source hash verified)",
+                "kernel_ms": avg_render_ms, "kernel_share_of_step": avg_render_ms / (total_ms / args.steps),
+                "algorithmic_flop_per_launch": steps_launch * flop_step}
+        # ---- CPU baseline: the oracle on a bounded sample of the same workload (about 10-30 s of host work)
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            stride = max(1, scene.ny // max(8, 2 * omp_threads()))
+            s_, dt = oracle_sample(scene, stride)
+            if dt < 5.0:
+                stride = max(1, stride // 4)
+                s_, dt = oracle_sample(scene, stride)
+            cpu = {"value": s_ / dt, "unit": UNIT, "cores": omp_threads(), "kind": "oracle",
+                   "sample": f"every {stride}th row of the {scene.nx}x{scene.ny} {args.workload} image "
+                             f"({s_} steps in {dt:.1f} s)"}
+        line["cpu_baseline"] = cpu
         if args.workload == "PB1":
             line["paper_geodesics_per_sec"] = PAPER_GEODESICS_PER_SEC      # other hardware, FP32: context only
         print(json.dumps(line))
     R.close()
     if world > 1:
         dist.destroy_process_group()
-
 
 def main():
     ap = argparse.ArgumentParser()
@@ -350,6 +375,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "PB1", "LC"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = one frame per rank (default), strong = one image sharded by tiles + all-reduce")
     ap.add_argument("--ref-row-stride", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

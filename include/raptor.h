@@ -10,6 +10,12 @@
  * the message.  "device" pointers are CUDA device memory of the current device, owned by the
  * caller; "host" pointers are ordinary host memory.  Calls taking a cuda_stream (a cudaStream_t
  * cast to void*, NULL = default stream) are asynchronous on that stream.
+ *
+ * Ordering: the asynchronous calls of one context share its scene data, its tile queue and its scratch
+ * buffers.  Issue them on ONE stream, or order the streams yourself (event / synchronise) before the next
+ * call on the same context; two calls of one context in flight at the same time are undefined.  The
+ * host-buffer call raptor_render_host runs on the context's own stream and orders itself after every
+ * earlier call made on that context (uploads included), then synchronises.
  */
 #ifndef RAPTOR_B200_H
 #define RAPTOR_B200_H
@@ -145,8 +151,10 @@ int raptor_light_curve(raptor_ctx *ctx, int32_t n_frames, double t_cam0, double 
 
 /* Multi-GPU sharding of one image: after this call raptor_render / raptor_spectrum /
  * raptor_render_host trace only the 8x4-pixel tiles rank, rank + world, rank + 2 world, ... (row-major tile
- * order) and leave every other pixel of the output buffers untouched.  Rays are independent, so the ranks'
- * images (zero-initialised by the caller) sum to the full image exactly.  Default (0, 1) = whole image. */
+ * order) and leave every other pixel of the caller's output buffers untouched.  Rays are independent, so the ranks'
+ * images (zero-initialised by the caller) sum to the full image exactly.  Where the library owns the image
+ * (raptor_spectrum with a NULL image, raptor_render_host) it zeroes it first, so fluxes are the shard's own and
+ * sum to the full flux.  Default (0, 1) = whole image. */
 int raptor_set_shard(raptor_ctx *ctx, int32_t rank, int32_t world);
 
 /* Render + flux reduction: d_flux_jy device [n_freq], F_k = 1e23 sum_pix I_k (fov/nx)(fov/ny) L^2/D^2 [Jy],
@@ -156,8 +164,9 @@ int raptor_spectrum(raptor_ctx *ctx, double *d_flux_jy, double *d_image_or_null,
 /* Flux reduction alone of an image already on the device. */
 int raptor_flux(raptor_ctx *ctx, const double *d_image, double *d_flux_jy, void *cuda_stream);
 
-/* End-to-end convenience with HOST buffers: render on the context's own stream, copy image
- * ([n_freq][ny][nx]), optional status / nsteps ([ny][nx]) and optional flux ([n_freq]) back, synchronise. */
+/* End-to-end convenience with HOST buffers: render on the context's own stream (after every earlier call on
+ * this context has finished, see "Ordering"), copy image ([n_freq][ny][nx]), optional status / nsteps ([ny][nx])
+ * and optional flux ([n_freq]) back, synchronise.  Under a shard the pixels of other ranks' tiles come back 0. */
 int raptor_render_host(raptor_ctx *ctx, double *h_image, int32_t *h_status, int32_t *h_nsteps, double *h_flux_jy);
 
 /* Diagnostics: trace n rays with given impact parameters (device arrays alpha[n], beta[n]) through the same
@@ -174,6 +183,13 @@ int raptor_eval_rhs(raptor_ctx *ctx, int32_t n, const double *d_XK, double *d_f,
  * states raptor_trace returns), d_out[n] out (device): 0 up to the integrator's truncation error.  d_ELQ_or_null
  * (device, [n][3]) receives the constants of motion E = -k_t, L = k_phi, Q of Eq. 38-40. */
 int raptor_null_norm(raptor_ctx *ctx, int32_t n, const double *d_XK, double *d_out, double *d_ELQ_or_null, void *cuda_stream);
+
+/* Null-condition monitor (Eq. 4): while d_null_max_or_null is set, raptor_render,
+ * raptor_render_disk and raptor_trace also evaluate g_mn k^m k^n at the new point of EVERY step and write its largest
+ * magnitude along each ray to d_null_max ([ny][nx], resp. [n]; device, caller-owned, must stay valid until unset).
+ * A ray whose norm peaked near the horizon and recovered is visible here, not in the end state.  The default kernels
+ * are unchanged; the monitoring variants cost about 5 % more.  NULL switches it off.  (raptor_light_curve ignores it.) */
+int raptor_set_null_monitor(raptor_ctx *ctx, double *d_null_max_or_null);
 
 /* Counters accumulated by every render / trace since creation (synchronises the context's work):
  * accepted RK4 steps, steps on which plasma was sampled, rays traced. */

@@ -24,7 +24,7 @@ STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 
 SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_render_disk",
            "raptor_line_profile", "raptor_set_camera_time", "raptor_set_window", "raptor_upload_snapshot",
            "raptor_light_curve", "raptor_spectrum", "raptor_flux",
-           "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_null_norm", "raptor_get_counters", "raptor_fp64_peak",
+           "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_null_norm", "raptor_set_null_monitor", "raptor_get_counters", "raptor_fp64_peak",
            "raptor_destroy", "raptor_last_error")
 
 
@@ -82,6 +82,7 @@ def lib():
         L.raptor_trace.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
         L.raptor_eval_rhs.argtypes = [vp, i32, vp, vp, vp]
         L.raptor_null_norm.argtypes = [vp, i32, vp, vp, vp, vp]
+        L.raptor_set_null_monitor.argtypes = [vp, vp]
         L.raptor_get_counters.argtypes = [vp, u64p, u64p, u64p]
         L.raptor_fp64_peak.argtypes = [i32, dp, dp]
         L.raptor_destroy.argtypes = [vp]
@@ -195,6 +196,10 @@ def raptor_eval_rhs(ctx, n, d_XK, d_f, stream=None):
 
 def raptor_null_norm(ctx, n, d_XK, d_out, d_ELQ=None, stream=None):
     _check(lib().raptor_null_norm(ctx, n, d_XK, d_out, d_ELQ, stream), ctx)
+
+
+def raptor_set_null_monitor(ctx, d_null_max=None):
+    _check(lib().raptor_set_null_monitor(ctx, d_null_max), ctx)
 
 
 def raptor_get_counters(ctx):
@@ -316,7 +321,7 @@ class Raptor:
         import torch
         torch.cuda.current_stream().synchronize()      # g may be a temporary
 
-    def trace(self, alpha, beta):
+    def trace(self, alpha, beta, monitor_null=False):
         import torch
         al = torch.as_tensor(np.asarray(alpha, dtype=np.float64)).cuda()
         be = torch.as_tensor(np.asarray(beta, dtype=np.float64)).cuda()
@@ -326,11 +331,21 @@ class Raptor:
         XK = torch.empty((n, 8), dtype=torch.float64, device="cuda")
         status = torch.empty((n,), dtype=torch.int32, device="cuda")
         nsteps = torch.empty((n,), dtype=torch.int32, device="cuda")
-        raptor_trace(self.ctx, n, al.data_ptr(), be.data_ptr(), I.data_ptr(), tau.data_ptr(), XK.data_ptr(),
-                     status.data_ptr(), nsteps.data_ptr(), _stream_ptr())
-        torch.cuda.synchronize()
-        return dict(I=I.cpu().numpy(), tau=tau.cpu().numpy(), XK=XK.cpu().numpy(),
-                    status=status.cpu().numpy(), nsteps=nsteps.cpu().numpy())
+        nmax = torch.zeros((n,), dtype=torch.float64, device="cuda") if monitor_null else None
+        if monitor_null:
+            raptor_set_null_monitor(self.ctx, nmax.data_ptr())
+        try:
+            raptor_trace(self.ctx, n, al.data_ptr(), be.data_ptr(), I.data_ptr(), tau.data_ptr(), XK.data_ptr(),
+                         status.data_ptr(), nsteps.data_ptr(), _stream_ptr())
+            torch.cuda.synchronize()
+        finally:
+            if monitor_null:
+                raptor_set_null_monitor(self.ctx, None)
+        out = dict(I=I.cpu().numpy(), tau=tau.cpu().numpy(), XK=XK.cpu().numpy(),
+                   status=status.cpu().numpy(), nsteps=nsteps.cpu().numpy())
+        if monitor_null:
+            out["null_max"] = nmax.cpu().numpy()
+        return out
 
     def eval_rhs(self, XK):
         import torch

@@ -15,6 +15,7 @@ using namespace raptor;
 
 struct raptor_ctx;
 static int ensure_scratch(raptor_ctx* ctx);
+static int mark(raptor_ctx* ctx, cudaStream_t s);
 
 struct raptor_ctx {
     raptor_params p;
@@ -36,6 +37,8 @@ struct raptor_ctx {
     double* d_scratch_flux = nullptr;
     size_t scratch_pixels = 0;
     cudaStream_t own_stream = nullptr;
+    double* d_null_max = nullptr;          // raptor_set_null_monitor: caller-owned output of the next render / trace calls
+    cudaEvent_t ev_last = nullptr;         // recorded after every asynchronous call: raptor_render_host orders itself after it
     char err[512] = {0};
 };
 
@@ -202,6 +205,7 @@ extern "C" int raptor_create(const raptor_params* p, raptor_ctx** out) {
     CKC(cudaGetDevice(&c->device));
     CKC(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
     CKC(cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking));
+    CKC(cudaEventCreateWithFlags(&c->ev_last, cudaEventDisableTiming));
     {
         // per-frequency constants of the transfer update: nu_k, nu_k^(1/6) (Eq. 43), c^2 / (2 h nu_k^3) (Eq. 45)
         double tab[3 * RAPTOR_MAX_FREQ];
@@ -238,16 +242,25 @@ extern "C" int raptor_upload_grid(raptor_ctx* ctx, const void* grid_host, uint64
     if (!ctx->d_grid) return fail(ctx, RAPTOR_EINVAL, "context has no grid");
     if (!grid_host || grid_bytes != ctx->grid_bytes) return fail(ctx, RAPTOR_EINVAL, "grid_bytes %llu != %zu", (unsigned long long)grid_bytes, ctx->grid_bytes);
     CK(ctx, cudaMemcpyAsync(ctx->d_grid, grid_host, ctx->grid_bytes, cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream));
+    return mark(ctx, (cudaStream_t)cuda_stream);
+}
+
+// Ordering rule (include/raptor.h): the asynchronous calls of one context share its scene data, tile queue and
+// scratch buffers, so the caller issues them on ONE stream (or orders its streams itself); every such call leaves
+// an event behind, and raptor_render_host, which runs on the context's own stream, waits for it.
+static int mark(raptor_ctx* ctx, cudaStream_t s) {
+    CK(ctx, cudaEventRecord(ctx->ev_last, s));
     return RAPTOR_OK;
 }
 
 static int run_rays(raptor_ctx* ctx, RenderOut& O, cudaStream_t s) {
     O.queue = ctx->d_queue;
     O.counters = ctx->d_counters;
+    if (O.frames <= 1) O.null_max = ctx->d_null_max;
     if (O.tile_stride == 0) { O.tile_offset = 0; O.tile_stride = 1; }
     CK(ctx, cudaMemsetAsync(ctx->d_queue, 0, sizeof(unsigned int), s));
     CK(ctx, launch_render(ctx->kp, ctx->p.plasma_model, O, ctx->sm_count, s));
-    return RAPTOR_OK;
+    return mark(ctx, s);
 }
 
 extern "C" int raptor_render(raptor_ctx* ctx, double* d_image, int32_t* d_status, int32_t* d_nsteps, void* cuda_stream) {
@@ -286,14 +299,14 @@ extern "C" int raptor_line_profile(raptor_ctx* ctx, const double* d_image, const
     if (nbins < 1 || nbins > 65535 || !(g_max > g_min)) return fail(ctx, RAPTOR_EINVAL, "need 1 <= nbins <= 65535 and g_max > g_min");
     const size_t npix = (size_t)ctx->p.nx * ctx->p.ny;
     if (ctx->profile_bins < nbins) {
-        if (ctx->d_profile_partial) cudaFree(ctx->d_profile_partial); cudaFree(ctx->d_lc_partial);
+        if (ctx->d_profile_partial) cudaFree(ctx->d_profile_partial);
         ctx->d_profile_partial = nullptr; ctx->profile_bins = 0;
         CK(ctx, cudaMalloc(&ctx->d_profile_partial, sizeof(double) * nbins * (size_t)flux_chunks(npix)));
         ctx->profile_bins = nbins;
     }
     const double area = (ctx->p.fov_M / ctx->p.nx) * (ctx->p.fov_M / ctx->p.ny);
     CK(ctx, launch_profile(d_image, d_redshift, npix, nbins, g_min, g_max, area, ctx->d_profile_partial, d_hist, (cudaStream_t)cuda_stream));
-    return RAPTOR_OK;
+    return mark(ctx, (cudaStream_t)cuda_stream);
 }
 
 // ---- slow-light movies and light curves (Sect. 5) -----------------------------------------
@@ -322,7 +335,7 @@ extern "C" int raptor_upload_snapshot(raptor_ctx* ctx, int64_t snapshot, const v
     if (snapshot < 0) return fail(ctx, RAPTOR_EINVAL, "snapshot index < 0");
     const size_t slot = (size_t)(snapshot % ctx->p.nt);
     CK(ctx, cudaMemcpyAsync((char*)ctx->d_grid + slot * one, host, one, cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream));
-    return RAPTOR_OK;
+    return mark(ctx, (cudaStream_t)cuda_stream);
 }
 
 // frames of a light curve rendered per launch: the image scratch is frames x n_freq x npix doubles
@@ -368,21 +381,30 @@ extern "C" int raptor_light_curve(raptor_ctx* ctx, int32_t n_frames, double t_ca
         O.image = ctx->d_scratch_image;
         if (nb == 1) { O.frames = 1; }       // single frame: the ordinary path with its own camera time
         const double keep = ctx->kp.t_cam;
+        double* keep_mon = ctx->d_null_max;          // the monitor buffer is one image: not for a batch of frames
+        ctx->d_null_max = nullptr;
         if (nb == 1) ctx->kp.t_cam = O.t_cam0;
         int rc = run_rays(ctx, O, s);
         ctx->kp.t_cam = keep;
+        ctx->d_null_max = keep_mon;
         if (rc) return rc;
         // the batch is [nb][n_freq][npix] = nb * n_freq planes: one deterministic reduction for all of them
         CK(ctx, launch_flux(ctx->d_scratch_image, npix, (int)(nb * p.n_freq), scale, ctx->d_lc_partial,
                             d_flux_jy + f0 * p.n_freq, s));
     }
-    return RAPTOR_OK;
+    return mark(ctx, s);
 }
 
 extern "C" int raptor_set_shard(raptor_ctx* ctx, int32_t rank, int32_t world) {
     if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
     if (world < 1 || rank < 0 || rank >= world) return fail(ctx, RAPTOR_EINVAL, "shard: need 0 <= rank < world");
     ctx->shard_rank = rank; ctx->shard_world = world;
+    return RAPTOR_OK;
+}
+
+extern "C" int raptor_set_null_monitor(raptor_ctx* ctx, double* d_null_max_or_null) {
+    if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    ctx->d_null_max = d_null_max_or_null;
     return RAPTOR_OK;
 }
 
@@ -393,7 +415,7 @@ extern "C" int raptor_flux(raptor_ctx* ctx, const double* d_image, double* d_flu
     const double L = ctx->kp.Lcm;
     const double scale = 1e23 * (p.fov_M / p.nx) * (p.fov_M / p.ny) * L * L / (p.D_src_cm * p.D_src_cm);
     CK(ctx, launch_flux(d_image, (size_t)p.nx * p.ny, p.n_freq, scale, ctx->d_partial, d_flux_jy, (cudaStream_t)cuda_stream));
-    return RAPTOR_OK;
+    return mark(ctx, (cudaStream_t)cuda_stream);
 }
 
 static int ensure_scratch(raptor_ctx* ctx) {
@@ -415,6 +437,9 @@ extern "C" int raptor_spectrum(raptor_ctx* ctx, double* d_flux_jy, double* d_ima
         int rc = ensure_scratch(ctx);
         if (rc) return rc;
         img = ctx->d_scratch_image;
+        // a shard writes only its own tiles: the rest of the scratch image must read as zero (raptor.h, raptor_set_shard)
+        if (ctx->shard_world > 1)
+            CK(ctx, cudaMemsetAsync(img, 0, (size_t)ctx->p.nx * ctx->p.ny * ctx->p.n_freq * sizeof(double), (cudaStream_t)cuda_stream));
     }
     int rc = raptor_render(ctx, img, nullptr, nullptr, cuda_stream);
     if (rc) return rc;
@@ -428,9 +453,15 @@ extern "C" int raptor_render_host(raptor_ctx* ctx, double* h_image, int32_t* h_s
     if (rc) return rc;
     const size_t npix = (size_t)ctx->p.nx * ctx->p.ny;
     cudaStream_t s = ctx->own_stream;
+    CK(ctx, cudaStreamWaitEvent(s, ctx->ev_last, 0));          // after every earlier call on this context (uploads, renders)
     int32_t *d_status = nullptr, *d_nsteps = nullptr;
     if (h_status) CK(ctx, cudaMallocAsync(&d_status, npix * sizeof(int32_t), s));
     if (h_nsteps) CK(ctx, cudaMallocAsync(&d_nsteps, npix * sizeof(int32_t), s));
+    if (ctx->shard_world > 1) {                                // pixels of other ranks' tiles read as zero
+        CK(ctx, cudaMemsetAsync(ctx->d_scratch_image, 0, npix * ctx->p.n_freq * sizeof(double), s));
+        if (d_status) CK(ctx, cudaMemsetAsync(d_status, 0, npix * sizeof(int32_t), s));
+        if (d_nsteps) CK(ctx, cudaMemsetAsync(d_nsteps, 0, npix * sizeof(int32_t), s));
+    }
     rc = raptor_render(ctx, ctx->d_scratch_image, d_status, d_nsteps, s);
     if (!rc && h_flux_jy) rc = raptor_flux(ctx, ctx->d_scratch_image, ctx->d_scratch_flux, s);
     if (!rc) {
@@ -520,6 +551,7 @@ extern "C" int raptor_destroy(raptor_ctx* ctx) {
     cudaFree(ctx->d_grid); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_counters);
     cudaFree(ctx->d_partial); cudaFree(ctx->d_profile_partial); cudaFree(ctx->d_lc_partial); cudaFree(ctx->d_scratch_image); cudaFree(ctx->d_scratch_flux);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);
     delete ctx;
     return RAPTOR_OK;
 }

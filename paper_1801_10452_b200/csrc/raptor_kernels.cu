@@ -36,7 +36,7 @@ cudaError_t launch_render(const KP& P, int model, const RenderOut& O, int sm_cou
     long long want = ((long long)O.ntiles + warps - 1) / warps;
     int grid = sm_count * per_sm;
     if (want < grid) grid = (int)(want > 0 ? want : 1);
-    const bool fullx = O.XK != nullptr;
+    const bool fullx = O.XK != nullptr || O.null_max != nullptr;
 #define RAPTOR_CASE_I(M, I) case I: return launch_model<M, I>(P, O, h1, multi, fullx, grid, block, stream);
 #define RAPTOR_CASE_M(M)                                                                          \
     case M:                                                                                       \

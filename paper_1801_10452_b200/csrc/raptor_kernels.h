@@ -33,6 +33,7 @@ struct RenderOut {
     int32_t* status;                // [npix]
     int32_t* nsteps;                // [npix]
     double* XK;                     // [npix][8] final state
+    double* null_max;               // [npix] max |g(k,k)| over the steps of the ray (Eq. 4), or NULL
     unsigned int frames;            // > 1: light-curve batch, image is [frames][n_freq][npix]; ntiles = frames * tiles_per_frame
     unsigned int tiles_per_frame;
     double t_cam0, dt_frame;        // camera time of frame f: t_cam0 + f dt_frame

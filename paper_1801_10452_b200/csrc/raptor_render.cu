@@ -17,6 +17,9 @@
 
 namespace raptor {
 
+#ifndef RAPTOR_FASTPATH
+#define RAPTOR_FASTPATH 0
+#endif
 #ifndef RAPTOR_REFRESH
 #define RAPTOR_REFRESH 15      // library exp / sincos at the base point every (RAPTOR_REFRESH + 1)-th step
 #endif
@@ -35,10 +38,12 @@ namespace raptor {
 // from the base point, stage 3 from stage 2 (offset (dl/2)^2 f_1) and the new base point from stage 4
 // (offset dl^2/6 (f_1 - 2 f_2 + f_3)), both of which are second / third order small.
 // --------------------------------------------------------------------------------------------
-template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG>
+// MON: also evaluate the null condition g_mn k^m k^n (Eq. 4) at the new point of every step and keep
+// its largest magnitude along the ray (8(a) a3 "null-condition check"); diagnostics, built with FULLX only.
+template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG, bool MON>
 __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta, double t_cam, double* __restrict__ sI,
                                           double* __restrict__ sTau, int sstride, double& I0, double& tau0,
-                                          double X[4], double K[4], int& status, int& nsteps, int& nsampled) {
+                                          double X[4], double K[4], int& status, int& nsteps, int& nsampled, double& null_max) {
     camera_ray(P, alpha, beta, X, K);
     X[0] = t_cam;
     double I = 0.0, tau = 0.0;
@@ -46,11 +51,13 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         for (int k = 0; k < P.n_freq; ++k) { sI[k * sstride] = 0.0; sTau[k * sstride] = 0.0; }
     }
     int n = 0, ns = 0, ncross = 0, st = S_RUNNING;
+    double nmax = 0.0;
     Geom G;
     { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
     for (;;) {
-        if (G.r < P.r_in) { st = S_CAPTURED; break; }                         // [A7]
-        if (G.r > P.r_out) { st = S_ESCAPED; break; }
+        // [A7]; r = r0 + e^x1 is positive (or +inf): compared on the integer pipe
+        if (pos_lt(G.r, P.r_in)) { st = S_CAPTURED; break; }
+        if (pos_lt(P.r_out, G.r)) { st = S_ESCAPED; break; }
         if (n >= P.max_steps) { st = S_MAXSTEPS; break; }
         if (P.use_tau_cutoff) {
             double tmin = tau;
@@ -67,6 +74,64 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         const double hl = 0.5 * dl;
         Geom Gs;                        // geometry of the last stage point: the new base point is reached from it
         double t1, t2;                  // new point minus that stage point (x1, x2)
+        bool have_G = false;            // the step already produced the geometry of the new point
+#if RAPTOR_FASTPATH
+        if (INTEG == I_RK4) {
+            // Straight-line step for the common case (9 of 10 steps): the polynomial tiers are fixed in advance --
+            // stage 2 and stage 4 from the base point with the tier-1 polynomials, stage 3 and the new point with the
+            // tier-0 ones -- so the whole step is one basic block the compiler can schedule (the stage-4 geometry
+            // overlaps the stage-3 right-hand side), and the bounds are VERIFIED afterwards on the integer pipe; a step
+            // that breaks one is redone by the tiered code below from the untouched (X, K, G).
+            const double ca = H1 ? kPI : 2.0 * kPI;
+            const double d12 = hl * K[1], d22 = hl * K[2], an2 = ca * d22;
+            // stage 4 lies about twice as far from the base point as stage 2: enter with a factor 2 of room
+            if (abs_hi(d12) < kTier1DHi - 0x00100000 && abs_hi(an2) < kTier1AHi - 0x00100000) {
+                double f0, f1, f2, f3, k0, k1, k2, k3, a0, a1, a2, a3, s0 = 0.0, s1, s2, s3 = 0.0;
+                Geom G2, G3, G4, Gn;
+                geodesic_rhs(P, G, K[0], K[1], K[2], K[3], f0, f1, f2, f3);
+                a0 = f0; a1 = f1; a2 = f2; a3 = f3;
+                k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
+                const double hh = hl * hl;
+                const double e1 = hh * f1, e2 = hh * f2, ane = ca * e2;
+                geom_shift_tier<H1, 5, 3, 3>(P, G, d12, d22, an2, G2);
+                geodesic_rhs(P, G2, k0, k1, k2, k3, f0, f1, f2, f3);
+                if (FULLX) { s0 = a0 + f0; s3 = a3 + f3; }
+                s1 = a1 + f1; s2 = a2 + f2;
+                a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
+                const double g1 = hl * f1, g2 = hl * f2;
+                k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
+                const double d14 = dl * k1, d24 = dl * k2, an4 = ca * d24;
+                geom_shift_tier<H1, 3, 1, 2>(P, G2, e1, e2, ane, G3);
+                geom_shift_tier<H1, 5, 3, 3>(P, G, d14, d24, an4, G4);
+                geodesic_rhs(P, G3, k0, k1, k2, k3, f0, f1, f2, f3);
+                if (FULLX) { s0 += f0; s3 += f3; }
+                s1 += f1; s2 += f2;
+                a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
+                k0 = fma(dl, f0, K[0]); k1 = fma(dl, f1, K[1]); k2 = fma(dl, f2, K[2]); k3 = fma(dl, f3, K[3]);
+                geodesic_rhs(P, G4, k0, k1, k2, k3, f0, f1, f2, f3);
+                a0 += f0; a1 += f1; a2 += f2; a3 += f3;
+                const double d6 = dl * (1.0 / 6.0);
+                const double u1 = dl * fma(d6, s1, -g1), u2 = dl * fma(d6, s2, -g2), anu = ca * u2;
+                const bool refresh = ((n + 1) & RAPTOR_REFRESH) == 0;          // warp-uniform
+                if (!refresh) geom_shift_tier<H1, 3, 1, 2>(P, G4, u1, u2, anu, Gn);
+                const bool ok = (abs_hi(e1) < kTier0Hi) & (abs_hi(ane) < kTier0Hi) & (abs_hi(d14) < kTier1DHi) &
+                                (abs_hi(an4) < kTier1AHi) & (abs_hi(u1) < kTier0Hi) & (abs_hi(anu) < kTier0Hi);
+                if (ok) {
+                    if (FULLX) { X[0] = fma(dl, fma(d6, s0, K[0]), X[0]); X[3] = fma(dl, fma(d6, s3, K[3]), X[3]); }
+                    X[1] = fma(dl, fma(d6, s1, K[1]), X[1]); X[2] = fma(dl, fma(d6, s2, K[2]), X[2]);
+                    K[0] = fma(d6, a0, K[0]); K[1] = fma(d6, a1, K[1]); K[2] = fma(d6, a2, K[2]); K[3] = fma(d6, a3, K[3]);
+                    if (!refresh) G = Gn;
+                    have_G = true;
+                } else {
+                    // rare (a few steps per ray next to the hole): the base-point geometry is re-evaluated rather than
+                    // kept in registers across the whole straight-line step
+                    Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T;
+                }
+            }
+        }
+        if (INTEG == I_RK4 && have_G) {
+        } else
+#endif
         if (INTEG == I_RK4) {
             double f0, f1, f2, f3;          // stage acceleration
             double k0, k1, k2, k3;          // stage wavevector
@@ -155,8 +220,15 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         // incremental from stage 4; re-evaluated with the library functions every (RAPTOR_REFRESH+1)-th step so
         // that the round-off of the increments cannot accumulate (n is warp-uniform: a tile's lanes start together)
         if ((n & RAPTOR_REFRESH) == 0) { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
+        else if (have_G) { }
         else if (INTEG == I_VERLET || INTEG == I_VERLET_C) G = Gs;
         else geom_shift<H1>(P, Gs, X[1], X[2], t1, t2, G);
+        if (MON) {
+            Met M;
+            met_eval(P, G, M);
+            const double kr = G.ex * K[1], kh = G.dth * K[2];
+            nmax = fmax(nmax, fabs(ks_dot(M, K[0], kr, kh, K[3], K[0], kr, kh, K[3])));
+        }
         if (MODEL == M_DISK) {
             // I = sum of g^p / r^2 over the counted crossings, tau = g of the first counted one
             double dI, gg;
@@ -166,7 +238,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
                 if (counted) { I += dI; if (ns == 0) tau = gg; ++ns; }
             }
         } else
-        if (MODEL != M_VACUUM && G.r >= P.r_in && G.r <= P.r_out) {            // [A8] end-point sample
+        if (MODEL != M_VACUUM && !pos_lt(G.r, P.r_in) && !pos_lt(P.r_out, G.r)) {   // [A8] end-point sample
             Plasma pl;
             if (plasma_sample<MODEL>(P, G, X, K[0], G.ex * K[1], G.dth * K[2], K[3], pl)) {
                 ++ns;
@@ -196,14 +268,14 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             }
         }
     }
-    I0 = I; tau0 = tau;
+    I0 = I; tau0 = tau; null_max = nmax;
     status = st; nsteps = n; nsampled = ns;
 }
 
 // --------------------------------------------------------------------------------------------
 // Persistent-warp driver: tiles of 8x4 pixels (render) or 32 consecutive rays (trace) from a global queue.
 // --------------------------------------------------------------------------------------------
-template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG>
+template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG, bool MON>
 __global__ void __launch_bounds__(MULTI ? RAPTOR_BLOCK_MULTI : RAPTOR_BLOCK, MULTI ? (RAPTOR_BLOCK * RAPTOR_MIN_BLOCKS) / RAPTOR_BLOCK_MULTI : RAPTOR_MIN_BLOCKS)
 k_render(const __grid_constant__ KP P, const RenderOut O) {
     extern __shared__ double smem[];
@@ -244,9 +316,9 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
             pix = (long long)iy * P.nx + ix;
         }
         if (active) {
-            double X[4], K[4], I0, tau0;
+            double X[4], K[4], I0, tau0, nmax;
             int status, n, ns;
-            trace_ray<MODEL, H1, MULTI, FULLX, INTEG>(P, alpha, beta, t_cam, sI, sTau, sstride, I0, tau0, X, K, status, n, ns);
+            trace_ray<MODEL, H1, MULTI, FULLX, INTEG, MON>(P, alpha, beta, t_cam, sI, sTau, sstride, I0, tau0, X, K, status, n, ns, nmax);
             steps += (unsigned)n; sampled += (unsigned)ns; rays += 1;
             const size_t npix = O.alpha ? (size_t)O.nrays : (size_t)P.nx * P.ny;
             if (O.image) {
@@ -258,6 +330,7 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
                 if (MULTI) { for (int k = 0; k < P.n_freq; ++k) O.tau[(size_t)k * npix + pix] = sTau[k * sstride]; }
                 else O.tau[pix] = tau0;
             }
+            if (MON && O.null_max) O.null_max[pix] = nmax;
             if (O.status) O.status[pix] = status;
             if (O.nsteps) O.nsteps[pix] = n;
             if (FULLX && O.XK) {
@@ -281,10 +354,10 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
     }
 }
 
-template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG>
+template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG, bool MON = false>
 static cudaError_t launch_one(const KP& P, const RenderOut& O, int grid, int block, cudaStream_t stream) {
     size_t smem = MULTI ? (size_t)2 * P.n_freq * block * sizeof(double) : 0;
-    auto kern = k_render<MODEL, H1, MULTI, FULLX, INTEG>;
+    auto kern = k_render<MODEL, H1, MULTI, FULLX, INTEG, MON>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -295,6 +368,10 @@ static cudaError_t launch_one(const KP& P, const RenderOut& O, int grid, int blo
 
 template <int MODEL, bool FULLX, int INTEG>
 static cudaError_t launch_hm(const KP& P, const RenderOut& O, bool h1, bool multi, int grid, int block, cudaStream_t s) {
+    if (FULLX && O.null_max) {           // per-step null monitor: the FULLX kernels with MON
+        if (h1) return multi ? launch_one<MODEL, true, true, FULLX, INTEG, FULLX>(P, O, grid, block, s) : launch_one<MODEL, true, false, FULLX, INTEG, FULLX>(P, O, grid, block, s);
+        return multi ? launch_one<MODEL, false, true, FULLX, INTEG, FULLX>(P, O, grid, block, s) : launch_one<MODEL, false, false, FULLX, INTEG, FULLX>(P, O, grid, block, s);
+    }
     if (h1) return multi ? launch_one<MODEL, true, true, FULLX, INTEG>(P, O, grid, block, s) : launch_one<MODEL, true, false, FULLX, INTEG>(P, O, grid, block, s);
     return multi ? launch_one<MODEL, false, true, FULLX, INTEG>(P, O, grid, block, s) : launch_one<MODEL, false, false, FULLX, INTEG>(P, O, grid, block, s);
 }
@@ -303,7 +380,7 @@ template <int MODEL, int INTEG>
 cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, int block, cudaStream_t s) {
     // the 3-D / slow-light sampler reads X^t, X^phi: always FULLX; the other models need them for the XK output only.
     // The second-order integrators (8(f) f1) are built in the FULLX form only.
-    if (MODEL == M_GRID3DT || fullx || INTEG != I_RK4) return launch_hm<MODEL, true, INTEG>(P, O, h1, multi, grid, block, s);
+    if (MODEL == M_GRID3DT || fullx || O.null_max || INTEG != I_RK4) return launch_hm<MODEL, true, INTEG>(P, O, h1, multi, grid, block, s);
     return launch_hm<MODEL, MODEL == M_GRID3DT || INTEG != I_RK4, INTEG>(P, O, h1, multi, grid, block, s);
 }
 

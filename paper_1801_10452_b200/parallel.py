@@ -51,3 +51,40 @@ def combine_tile_shards(image: torch.Tensor) -> torch.Tensor:
     if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
         dist.all_reduce(image, op=dist.ReduceOp.SUM)
     return image
+
+
+def world_info():
+    """(rank, world) of the initialised process group, (0, 1) without one."""
+    if dist.is_available() and dist.is_initialized():
+        return dist.get_rank(), dist.get_world_size()
+    return 0, 1
+
+
+def frame_of_rank(scene, rank: int, frame_dt: float = 2.5, seed_stride: int = 1):
+    """Weak scaling = a movie, one frame per rank: a slow-light scene gets its own camera time
+    t_cam + rank * frame_dt, a fast-light grid scene its own snapshot (the seeded generator with seed + rank), an
+    analytic scene is stationary (every frame is the same image).  Pure bookkeeping on the scene description."""
+    from dataclasses import replace
+    if rank == 0:
+        return scene
+    if getattr(scene, "slow_light", 0):
+        return replace(scene, t_cam=scene.t_cam + rank * frame_dt)
+    if getattr(scene, "grid", None) is not None and scene.nt == 1 and scene.n3 == 1:
+        from . import scenes
+        g = scenes.synthetic_grid(seed=1801 + seed_stride * rank, a=scene.a, h=scene.mks_h, n1=scene.n1, n2=scene.n2)
+        return replace(scene, grid=g[0])
+    if getattr(scene, "grid", None) is not None:
+        return replace(scene, snapshot=(scene.snapshot + rank) % scene.nt)
+    return scene
+
+
+def strong_step(render_shard, image: torch.Tensor, reduce_flux):
+    """One strong-scaling step of ONE image over all ranks: every rank traces its interleaved
+    tiles (raptor_set_shard(rank, world) was called on its context) into a zeroed image, one all-reduce(SUM) of the
+    image makes it whole on every rank (disjoint support: exact), and the flux is reduced from the whole image.
+    ``render_shard(image)`` and ``reduce_flux(image)`` are the two C-ABI calls; this function is what
+    ``bench.py --scaling strong`` times and what the world-size-2 gloo test drives with a fake renderer."""
+    image.zero_()
+    render_shard(image)
+    combine_tile_shards(image)
+    return reduce_flux(image)

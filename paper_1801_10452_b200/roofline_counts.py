@@ -1,0 +1,133 @@
+"""FP64 work per accepted integrator step of the shipped kernels: the numerator of bench.py's roofline.
+
+The counts are MEASURED, not typed in: one ncu pass per workload W over the same bench command,
+
+    python bench.py --workload W --steps 1 --warmup 3 --no-cpu-baseline > gpurun_out/bench_W.json   (must exit 0) &&
+    ncu --metrics smsp__sass_thread_inst_executed_op_dfma_pred_on.sum,smsp__sass_thread_inst_executed_op_dmul_pred_on.sum,\
+smsp__sass_thread_inst_executed_op_dadd_pred_on.sum,smsp__inst_executed_pipe_fp64.sum,smsp__inst_executed.sum,\
+smsp__thread_inst_executed.sum,gpu__time_duration.sum,sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active,\
+dram__bytes_read.sum,dram__bytes_write.sum \
+        --clock-control none -k regex:k_render -s 3 -c 1 --csv --log-file gpurun_out/flops_W.csv \
+        python bench.py --workload W --steps 1 --warmup 3 --no-cpu-baseline
+
+and then, here,
+
+    python -m paper_1801_10452_b200.roofline_counts gpurun_out profiles/fp64_inst_per_step.json
+
+divides the thread-level counters of that k_render launch by the accepted steps of the image (the library's own
+counter, printed by the plain run as steps_per_image) and stamps the result with the SHA-256 of the kernel sources
+(csrc/*).  bench.py recomputes that hash from the sources it runs and reports roofline = null with the reason when
+they differ: a kernel edit cannot silently falsify the roofline fraction.
+"""
+from __future__ import annotations
+
+import csv
+import hashlib
+import json
+import os
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+DEFAULT_JSON = os.path.join(os.path.dirname(HERE), "profiles", "fp64_inst_per_step.json")
+WORKLOADS = ("C0", "C1", "C2", "C3", "C4", "PB1", "PB1F32", "LC")
+
+METRICS = {
+    "dfma": "smsp__sass_thread_inst_executed_op_dfma_pred_on.sum",
+    "dmul": "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum",
+    "dadd": "smsp__sass_thread_inst_executed_op_dadd_pred_on.sum",
+    "ffma": "smsp__sass_thread_inst_executed_op_ffma_pred_on.sum",
+    "fmul": "smsp__sass_thread_inst_executed_op_fmul_pred_on.sum",
+    "fadd": "smsp__sass_thread_inst_executed_op_fadd_pred_on.sum",
+    "fp64_pipe_warp_inst": "smsp__inst_executed_pipe_fp64.sum",
+    "warp_inst": "smsp__inst_executed.sum",
+    "thread_inst": "smsp__thread_inst_executed.sum",
+    "kernel_ns": "gpu__time_duration.sum",
+    "fp64_pipe_pct": "sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active",
+    "dram_read_bytes": "dram__bytes_read.sum",
+    "dram_write_bytes": "dram__bytes_write.sum",
+}
+
+
+def csrc_sha256() -> str:
+    """SHA-256 over the kernel sources (names and contents, sorted): identifies the kernel the counts belong to."""
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(CSRC)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            h.update(name.encode())
+            with open(os.path.join(CSRC, name), "rb") as fh:
+                h.update(fh.read())
+    return h.hexdigest()
+
+
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "nsecond": 1.0, "usecond": 1e3, "msecond": 1e6, "second": 1e9,
+         "ns": 1.0, "us": 1e3, "ms": 1e6, "s": 1e9}
+
+
+def parse_ncu_csv(path: str) -> dict:
+    """Metric name -> value (bytes, ns, counts) of the FIRST profiled launch in an ncu --csv log."""
+    with open(path, newline="") as fh:
+        lines = [ln for ln in fh if ln.startswith('"')]
+    rows = list(csv.reader(lines))
+    head = rows[0]
+    i_name, i_unit, i_val, i_id = head.index("Metric Name"), head.index("Metric Unit"), head.index("Metric Value"), head.index("ID")
+    first = rows[1][i_id]
+    out = {}
+    for r in rows[1:]:
+        if r[i_id] != first:
+            continue
+        out[r[i_name]] = float(r[i_val].replace(",", "")) * _UNIT.get(r[i_unit], 1.0)
+    return out
+
+
+def collect(run_dir: str) -> dict:
+    table = {}
+    for w in WORKLOADS:
+        f_csv, f_json = os.path.join(run_dir, f"flops_{w}.csv"), os.path.join(run_dir, f"bench_{w}.json")
+        if not (os.path.exists(f_csv) and os.path.exists(f_json)):
+            continue
+        with open(f_json) as fh:
+            bench = json.loads(fh.read().strip().splitlines()[-1])
+        steps = float(bench["steps_per_image"])
+        m = parse_ncu_csv(f_csv)
+        row = {"steps_per_launch": steps}
+        for key, name in METRICS.items():
+            if name in m:
+                row[key] = m[name] if key in ("kernel_ns", "fp64_pipe_pct", "dram_read_bytes", "dram_write_bytes") else m[name] / steps
+        table[w] = row
+    return table
+
+
+def load(path: str = DEFAULT_JSON):
+    """(table, None) if the committed counts belong to the sources in this tree, else (None, reason)."""
+    if not os.path.exists(path):
+        return None, f"{os.path.relpath(path, os.path.dirname(HERE))} is missing"
+    with open(path) as fh:
+        doc = json.load(fh)
+    have = csrc_sha256()
+    if doc.get("csrc_sha256") != have:
+        return None, (f"profiles/fp64_inst_per_step.json was measured on csrc {str(doc.get('csrc_sha256'))[:12]}, "
+                      f"the sources here hash to {have[:12]}: re-run the ncu pass (paper_1801_10452_b200/roofline_counts.py)")
+    return doc["per_step"], None
+
+
+def main(argv):
+    run_dir = argv[1] if len(argv) > 1 else "gpurun_out"
+    out = argv[2] if len(argv) > 2 else DEFAULT_JSON
+    table = collect(run_dir)
+    if not table:
+        raise SystemExit(f"no flops_<W>.csv + bench_<W>.json pairs under {run_dir}")
+    doc = {"csrc_sha256": csrc_sha256(),
+           "what": "thread-level executed FP64 instructions of one k_render launch / accepted steps of that launch; "
+                   "flop = 2 dfma + dmul + dadd; fp64_pipe_warp_inst = warp-level instructions issued to the FP64 pipe "
+                   "(arithmetic + DSETP etc.); kernel_ns, dram bytes: that launch under ncu (cold cache, serialised)",
+           "command": "see the docstring of paper_1801_10452_b200/roofline_counts.py",
+           "per_step": table}
+    with open(out, "w") as fh:
+        json.dump(doc, fh, indent=1, sort_keys=True)
+        fh.write("\n")
+    print(json.dumps(doc, indent=1, sort_keys=True))
+
+
+if __name__ == "__main__":
+    main(sys.argv)

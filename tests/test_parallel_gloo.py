@@ -27,7 +27,24 @@ def _worker(rank, world, port, nx, ny, out):
         combined = parallel.combine_tile_shards(mine.clone())
         t, u = parallel.aggregate(10.0 + rank, float((owner == rank).sum()))
         frames = list(parallel.frames_of_rank(7, rank, world))
-        out.put((rank, bool(torch.equal(combined, full)), t, u, frames))
+        # the exact function bench.py --scaling strong times, with a fake renderer standing in for raptor_render
+        # under raptor_set_shard(rank, world): it writes this rank's tiles only and leaves the rest untouched
+        calls = []
+
+        def fake_render_shard(img):
+            assert float(img.abs().sum()) == 0.0            # strong_step zeroed it first
+            img[owner == rank] = full[owner == rank]
+            calls.append("render")
+
+        def fake_flux(img):
+            calls.append("flux")
+            return img.sum()
+
+        stale = torch.full_like(full, 99.0)                 # last step's image: must not leak into this one
+        flux = parallel.strong_step(fake_render_shard, stale, fake_flux)
+        strong_ok = bool(torch.equal(stale, full)) and float(flux) == float(full.sum()) and calls == ["render", "flux"]
+        assert parallel.world_info() == (rank, world)
+        out.put((rank, bool(torch.equal(combined, full)) and strong_ok, t, u, frames))
     finally:
         dist.destroy_process_group()
 
@@ -61,3 +78,18 @@ def test_tiles_are_dealt_exactly_once():
         counts = torch.bincount(owner.flatten(), minlength=world)
         if parallel.n_tiles(nx, ny) >= 4 * world:
             assert counts.max() - counts.min() <= 2 * 32 + nx     # balanced to within a couple of tiles / ragged edge
+
+
+def test_frame_of_rank_gives_every_rank_its_own_frame():
+    from paper_1801_10452_b200 import scenes
+    c4 = scenes.config_C4(nx=8, n1=8, n2=8, n3=4, nt=4)
+    ts = [parallel.frame_of_rank(c4, r).t_cam for r in range(4)]
+    assert ts[0] == c4.t_cam and all(b - a == 2.5 for a, b in zip(ts, ts[1:]))          # own camera time
+    c2 = scenes.config_C2(nx=8, n1=16, n2=16)
+    g = [parallel.frame_of_rank(c2, r).grid for r in range(3)]
+    assert g[0] is c2.grid and g[1].shape == c2.grid.shape
+    assert not (g[1] == g[0]).all() and not (g[2] == g[1]).all() and (g[1][..., 0] > 0).all()   # own seeded snapshot
+    fast = scenes.config_C4(nx=8, n1=8, n2=8, n3=4, nt=4, slow_light=False)
+    assert [parallel.frame_of_rank(fast, r).snapshot for r in range(3)] == [2, 3, 0]
+    c1 = scenes.config_C1(8)
+    assert parallel.frame_of_rank(c1, 3) is c1                                          # stationary analytic scene
