@@ -37,7 +37,8 @@
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/oracle.py does it).
  */
 #include <math.h>
-#include <tgmath.h>
+#include <tgmath.h>   /* type-generic sin, exp, ... : the float functions when real = float */
+#undef I              /* <complex.h>'s imaginary unit, pulled in by <tgmath.h>: I is the intensity here */
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
