@@ -42,11 +42,16 @@ FP64_PEAK_NOMINAL_TFLOPS = 148 * 4 * 16 * 2 * 1.965e9 / 1e12
 PAPER_GEODESICS_PER_SEC = {"GTX 1080, OpenACC, single precision": 104900.0, "i7-6950X 10 cores, OpenMP, single precision": 10707.0}
 
 
-LC_FRAMES, LC_DT = 32, 2.5      # workload LC: frames per light curve, camera-time spacing [M]
+LC_DT = 2.5      # workloads LC (32 frames per light curve) and C3B (8 spectra): camera-time spacing [M]
 
 
 def build_scene(workload: str):
     from paper_1801_10452_b200 import scenes
+    if workload == "C3B":
+        # a batch of C3 spectra (256^2 x 32 frequencies each) traced by ONE launch: a single 256^2 frame is one wave of
+        # 2,048 warps whose time is its longest ray's; batching is what fills the GPU
+        from dataclasses import replace
+        return replace(scenes.config("C3"), name="C3B")
     if workload == "LC":
         # slow-light light curve (Sect. 5): 256^2 pixels, the paper's four VLBI frequencies, 16 snapshots
         from dataclasses import replace
@@ -108,7 +113,7 @@ class ClockSampler:
 def oracle_sample(scene, row_stride, repeats=1):
     """Times the oracle, as it stands, on every row_stride-th image row of the workload (host cores)."""
     from oracle import oracle
-    o = oracle.Oracle(scene)
+    o = oracle.Oracle(scene, dtype="f32" if getattr(scene, "precision", 0) == 1 else "f64")
     t0 = time.perf_counter()
     steps = 0
     for _ in range(repeats):
@@ -145,7 +150,7 @@ def run_reference(args):
               f"({len(range(stride // 2, scene.ny, stride))} rows on {omp_threads()} threads)")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f32" if scene.precision == 1 else "f64", "data": "synthetic",
             "config": {"workload": args.workload, "pixels": [scene.nx, scene.ny], "n_freq": scene.n_freq,
                        "note": "CPU oracle (oracle/raptor_oracle.c) as it stands, OpenMP over image rows"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": omp_threads(), "kind": "oracle", "sample": sample},
@@ -172,7 +177,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     binding.lib()
 
-    lc = args.workload == "LC"
+    lc = args.workload in ("LC", "C3B")
+    LC_FRAMES = {"LC": 32, "C3B": 8}.get(args.workload, 1)
     strong = args.scaling == "strong" and world > 1
     if strong and lc:
         raise SystemExit("--scaling strong shards one image by tiles; a light curve shards by frames")
@@ -302,7 +308,7 @@ def run_ours(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "strong" if strong else "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f32" if scene.precision == 1 else "f64", "data": "synthetic",
             "config": {"workload": args.workload, "pixels": [scene.nx, scene.ny], "n_freq": scene.n_freq,
                        "spin": scene.a, "incl_deg": scene.incl_deg, "plasma_model": scene.plasma_model,
                        "grid": [scene.nt, scene.n1, scene.n2, scene.n3], "l2": "flushed between timed iterations",
@@ -328,6 +334,20 @@ def run_ours(args):
         if row is None:
             line["roofline"] = None
             line["roofline_unavailable"] = why or f"no ncu counts for workload {args.workload} in profiles/fp64_inst_per_step.json"
+        elif scene.precision == 1:
+            # the single-precision kernel: FP32 FMA pipe, 128 lanes per SM; peak derived from unit counts and clocks
+            flop_step = 2.0 * row["ffma"] + row["fmul"] + row["fadd"]
+            steps_launch = steps_done / args.steps
+            achieved = steps_launch * flop_step / (avg_render_ms * 1e-3) / 1e12
+            peak32 = 148 * 128 * 2 * 1.965e9 / 1e12
+            line["roofline"] = {
+                "bound": "alu", "kernel": "k_render_f32", "achieved": achieved, "peak": peak32, "unit": "TFLOP/s",
+                "frac": achieved / peak32, "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (no measured FP32 peak)",
+                "traffic": (row.get("dram_read_bytes", 0.0) + row.get("dram_write_bytes", 0.0)) if "dram_read_bytes" in row else None,
+                "fp32_inst_per_step": {"ffma": row["ffma"], "fmul": row["fmul"], "fadd": row["fadd"]},
+                "counts_source": "profiles/fp64_inst_per_step.json (ncu, source hash verified)",
+                "kernel_ms": avg_render_ms, "kernel_share_of_step": avg_render_ms / (total_ms / args.steps),
+                "algorithmic_flop_per_launch": steps_launch * flop_step}
         else:
             flop_step = 2.0 * row["dfma"] + row["dmul"] + row["dadd"]
             steps_launch = steps_done / args.steps
@@ -361,7 +381,7 @@ def run_ours(args):
                    "sample": f"every {stride}th row of the {scene.nx}x{scene.ny} {args.workload} image "
                              f"({s_} steps in {dt:.1f} s)"}
         line["cpu_baseline"] = cpu
-        if args.workload == "PB1":
+        if args.workload in ("PB1", "PB1F32"):
             line["paper_geodesics_per_sec"] = PAPER_GEODESICS_PER_SEC      # other hardware, FP32: context only
         print(json.dumps(line))
     R.close()
@@ -374,7 +394,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "PB1", "LC"])
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "PB1", "PB1F32", "LC", "C3B"])
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = one frame per rank (default), strong = one image sharded by tiles + all-reduce")
     ap.add_argument("--ref-row-stride", type=int, default=0)

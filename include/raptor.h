@@ -26,7 +26,7 @@
 extern "C" {
 #endif
 
-#define RAPTOR_ABI_VERSION 1u
+#define RAPTOR_ABI_VERSION 2u
 
 enum {
     RAPTOR_OK = 0,
@@ -99,6 +99,11 @@ typedef struct {
     int32_t slow_light;        /* 1: interpolate between snapshots at the ray's coordinate time */
     int32_t snapshot;          /* fast light: snapshot index used */
     int32_t te_model;          /* 0: constant tp_over_te; 1: Eq. 47, model[0] = R_low, model[1] = R_high (grids) */
+    int32_t precision;         /* 0: FP64 (the contract).  1: FP32, the paper's own performance configuration only (Table B.1,
+                                  PAPER.md:638-647 "Single precision: yes"): plasma_model = GRID2D, integrator = 3 (RK2),
+                                  step_policy = 1, n_freq = 1, k2_mode = 0, te_model = 0; raptor_render / raptor_spectrum /
+                                  raptor_flux / raptor_render_host / raptor_trace; images are still written as float64 */
+    int32_t reserved_;         /* 0 */
 } raptor_params;
 
 /* Validates and copies *p, uploads frequencies and grid.  *out is NULL on failure (then
@@ -198,6 +203,14 @@ int raptor_get_counters(raptor_ctx *ctx, uint64_t *total_steps, uint64_t *sample
 /* Measures the FP64 FMA peak of the current device with independent DFMA chains on all SMs:
  * *tflops = 2 * FMAs / time.  iters = chain length per thread (e.g. 1<<16). Synchronous. */
 int raptor_fp64_peak(int32_t iters, double *tflops, double *ms);
+
+/* Issue rate of the FP64 pipe by operand form (independent chains on all SMs, 8 warps per sub-partition):
+ * form 0 fma(x, imm, imm); 1 fma(y, z, x) = three different register sources; 2 fma(x, y, x); 3 x * y; 4 x + z.
+ * *warp_inst_per_sec = warp-level instructions per second over the whole device; *sm_clock_hz (may be NULL) = the
+ * device's nominal SM clock, so that cycles per instruction per sub-partition = 4 SMs clock / rate.  Synchronous.
+ * On B200 a DFMA with three different register sources issues every 3.2 cycles, every other form every 2.06
+ * (DESIGN.md 5.1): the bound of a kernel depends on its operand forms, not only on its instruction count. */
+int raptor_fp64_probe(int32_t form, int32_t iters, double *warp_inst_per_sec, double *sm_clock_hz);
 
 int raptor_destroy(raptor_ctx *ctx);
 

@@ -16,91 +16,120 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "raptor_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
+_LIB_F32 = os.path.join(_HERE, "liboracle_f32.so")
 
 STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 5: "NONFINITE"}
 
 
-def build(force: bool = False) -> str:
-    """gcc -O2 -ffp-contract=off (no FMA contraction) -fopenmp, rows-only parallelism."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-Wall", "-shared", "-fPIC",
-               "-o", _LIB, _SRC, "-lm"]
-        subprocess.check_call(cmd)
-    return _LIB
+def build(force: bool = False, dtype: str = "f64") -> str:
+    """gcc -O2 -ffp-contract=off (no FMA contraction) -fopenmp, rows-only parallelism.  dtype "f32": the SAME source
+    with real = float and single-precision constants (Table B.1 of the paper: "Single precision: yes")."""
+    out = _LIB if dtype == "f64" else _LIB_F32
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-Wall", "-shared", "-fPIC"]
+        if dtype == "f32":
+            cmd += ["-DORC_REAL=float", "-fsingle-precision-constant"]
+        subprocess.check_call(cmd + ["-o", out, _SRC, "-lm"])
+    return out
 
 
-class OrcParams(C.Structure):
-    _fields_ = [
-        ("a", C.c_double), ("mks_h", C.c_double), ("mks_r0", C.c_double), ("mass", C.c_double),
-        ("r_cam", C.c_double), ("incl_deg", C.c_double), ("fov_M", C.c_double), ("t_cam", C.c_double),
-        ("M_bh_g", C.c_double), ("D_src_cm", C.c_double), ("M_unit_g", C.c_double),
-        ("step_c", C.c_double), ("step_min", C.c_double), ("step_max", C.c_double),
-        ("eps", C.c_double), ("delta", C.c_double), ("eps_polar", C.c_double),
-        ("r_stop_in_factor", C.c_double), ("r_stop_out_factor", C.c_double), ("tau_cutoff", C.c_double),
-        ("model", C.c_double * 16),
-        ("tp_over_te", C.c_double), ("gamma_ad", C.c_double),
-        ("x1_min", C.c_double), ("x1_max", C.c_double), ("t0", C.c_double), ("dt_snap", C.c_double),
-        ("freq_hz", C.POINTER(C.c_double)),
-        ("grid", C.c_void_p),
-        ("nx", C.c_int32), ("ny", C.c_int32), ("integrator", C.c_int32), ("step_policy", C.c_int32),
-        ("max_steps", C.c_int32), ("n_freq", C.c_int32), ("plasma_model", C.c_int32), ("k2_mode", C.c_int32),
-        ("n1", C.c_int32), ("n2", C.c_int32), ("n3", C.c_int32), ("nt", C.c_int32),
-        ("grid_dtype", C.c_int32), ("slow_light", C.c_int32), ("snapshot", C.c_int32), ("te_model", C.c_int32),
-    ]
+class _Types:
+    """ctypes mirror of the oracle's types for one working precision (real = double or float)."""
+
+    def __init__(self, dtype: str):
+        assert dtype in ("f64", "f32"), dtype
+        self.dtype = dtype
+        R = self.REAL = C.c_double if dtype == "f64" else C.c_float
+        self.np_real = np.float64 if dtype == "f64" else np.float32
+        self.D4 = R * 4
+        self.D44 = (R * 4) * 4
+        self.D444 = ((R * 4) * 4) * 4
+
+        class OrcParams(C.Structure):
+            _fields_ = [
+                ("a", R), ("mks_h", R), ("mks_r0", R), ("mass", R),
+                ("r_cam", R), ("incl_deg", R), ("fov_M", R), ("t_cam", R),
+                ("M_bh_g", C.c_double), ("D_src_cm", C.c_double), ("M_unit_g", C.c_double),     # beyond float range
+                ("step_c", R), ("step_min", R), ("step_max", R),
+                ("eps", R), ("delta", R), ("eps_polar", R),
+                ("r_stop_in_factor", R), ("r_stop_out_factor", R), ("tau_cutoff", R),
+                ("model", R * 16),
+                ("tp_over_te", R), ("gamma_ad", R),
+                ("x1_min", R), ("x1_max", R), ("t0", R), ("dt_snap", R),
+                ("freq_hz", C.POINTER(R)),
+                ("grid", C.c_void_p),
+                ("nx", C.c_int32), ("ny", C.c_int32), ("integrator", C.c_int32), ("step_policy", C.c_int32),
+                ("max_steps", C.c_int32), ("n_freq", C.c_int32), ("plasma_model", C.c_int32), ("k2_mode", C.c_int32),
+                ("n1", C.c_int32), ("n2", C.c_int32), ("n3", C.c_int32), ("nt", C.c_int32),
+                ("grid_dtype", C.c_int32), ("slow_light", C.c_int32), ("snapshot", C.c_int32), ("te_model", C.c_int32),
+            ]
+
+        class RayResult(C.Structure):
+            _fields_ = [("status", C.c_int32), ("nsteps", C.c_int32), ("nsampled", C.c_int32), ("pad_", C.c_int32),
+                        ("null_max", R), ("X", R * 4), ("K", R * 4)]
+
+        self.OrcParams, self.RayResult = OrcParams, RayResult
+        L = self.lib = C.CDLL(build(dtype=dtype))
+        L.orc_sizeof_params.restype = C.c_size_t
+        L.orc_sizeof_ray_result.restype = C.c_size_t
+        assert L.orc_sizeof_params() == C.sizeof(OrcParams), (L.orc_sizeof_params(), C.sizeof(OrcParams))
+        assert L.orc_sizeof_ray_result() == C.sizeof(RayResult)
+        PP, D4, D44 = C.POINTER(OrcParams), self.D4, self.D44
+        L.orc_null_norm.restype = R
+        L.orc_step_size.restype = R
+        L.orc_planck.restype = R
+        L.orc_planck.argtypes = [R, R]
+        L.orc_emissivity.restype = R
+        L.orc_emissivity.argtypes = [R] * 5 + [C.c_int]
+        L.orc_bessel_k2.restype = R
+        L.orc_bessel_k2.argtypes = [R]
+        L.orc_horizon.restype = R
+        L.orc_r_isco.restype = R
+        L.orc_r_isco.argtypes = [R]
+        L.orc_line_profile.argtypes = [PP, C.c_void_p, C.c_void_p, C.c_int, R, R, C.c_void_p]
+        L.orc_transfer_update.argtypes = [C.POINTER(R), C.POINTER(R)] + [R] * 5
+        L.orc_mks_theta.argtypes = [R, R] + [C.POINTER(R)] * 3
+        L.orc_x2_of_theta.argtypes = [R, R, R, C.POINTER(R)]
+        L.orc_metric_ks.argtypes = [R] * 4 + [D44]
+        L.orc_metric_ks_inv.argtypes = [R] * 4 + [D44]
+        L.orc_camera_ab.argtypes = [PP, R, R, D4, D4]
+        L.orc_pixel_ab.argtypes = [PP, C.c_int, C.c_int, C.POINTER(R), C.POINTER(R)]
+        L.orc_rk4_step.argtypes = [PP, D4, D4, R]
+        L.orc_verlet_step.argtypes = [PP, D4, D4, R, C.c_int]
+        L.orc_rk2_step.argtypes = [PP, D4, D4, R]
+        L.orc_step.argtypes = [PP, D4, D4, R]
+        L.orc_transfer.argtypes = [PP, D4, D4, R, C.c_void_p, C.c_void_p]
+        L.orc_trace_ray.argtypes = [PP, R, R, C.c_void_p, C.c_void_p, C.POINTER(RayResult), C.c_void_p, C.c_int, C.c_int]
 
 
-class RayResult(C.Structure):
-    _fields_ = [("status", C.c_int32), ("nsteps", C.c_int32), ("nsampled", C.c_int32), ("pad_", C.c_int32),
-                ("null_max", C.c_double), ("X", C.c_double * 4), ("K", C.c_double * 4)]
+_types: dict = {}
 
 
-_lib = None
-_D4 = C.c_double * 4
-_D44 = (C.c_double * 4) * 4
-_D444 = ((C.c_double * 4) * 4) * 4
+def types(dtype: str = "f64") -> _Types:
+    if dtype not in _types:
+        _types[dtype] = _Types(dtype)
+    return _types[dtype]
 
 
-def lib():
-    global _lib
-    if _lib is None:
-        _lib = C.CDLL(build())
-        assert _lib.orc_sizeof_params() == C.sizeof(OrcParams)
-        assert _lib.orc_sizeof_ray_result() == C.sizeof(RayResult)
-        _lib.orc_null_norm.restype = C.c_double
-        _lib.orc_step_size.restype = C.c_double
-        _lib.orc_planck.restype = C.c_double
-        _lib.orc_planck.argtypes = [C.c_double, C.c_double]
-        _lib.orc_emissivity.restype = C.c_double
-        _lib.orc_emissivity.argtypes = [C.c_double] * 5 + [C.c_int]
-        _lib.orc_bessel_k2.restype = C.c_double
-        _lib.orc_bessel_k2.argtypes = [C.c_double]
-        _lib.orc_horizon.restype = C.c_double
-        _lib.orc_r_isco.restype = C.c_double
-        _lib.orc_r_isco.argtypes = [C.c_double]
-        _lib.orc_line_profile.argtypes = [C.POINTER(OrcParams), C.c_void_p, C.c_void_p, C.c_int, C.c_double,
-                                          C.c_double, C.c_void_p]
-        _lib.orc_sizeof_params.restype = C.c_size_t
-        _lib.orc_transfer_update.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)] + [C.c_double] * 5
-        _lib.orc_mks_theta.argtypes = [C.c_double, C.c_double] + [C.POINTER(C.c_double)] * 3
-        _lib.orc_x2_of_theta.argtypes = [C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]
-        _lib.orc_metric_ks.argtypes = [C.c_double] * 4 + [_D44]
-        _lib.orc_metric_ks_inv.argtypes = [C.c_double] * 4 + [_D44]
-        _lib.orc_camera_ab.argtypes = [C.POINTER(OrcParams), C.c_double, C.c_double, _D4, _D4]
-        _lib.orc_rk4_step.argtypes = [C.POINTER(OrcParams), _D4, _D4, C.c_double]
-        _lib.orc_verlet_step.argtypes = [C.POINTER(OrcParams), _D4, _D4, C.c_double, C.c_int]
-        _lib.orc_rk2_step.argtypes = [C.POINTER(OrcParams), _D4, _D4, C.c_double]
-        _lib.orc_step.argtypes = [C.POINTER(OrcParams), _D4, _D4, C.c_double]
-        _lib.orc_trace_ray.argtypes = [C.POINTER(OrcParams), C.c_double, C.c_double, C.c_void_p, C.c_void_p,
-                                       C.POINTER(RayResult), C.c_void_p, C.c_int, C.c_int]
-    return _lib
+def lib(dtype: str = "f64"):
+    return types(dtype).lib
+
+
+# the float64 structures under their old names
+def __getattr__(name):
+    if name in ("OrcParams", "RayResult"):
+        return getattr(types("f64"), name)
+    raise AttributeError(name)
 
 
 class Oracle:
     """Holds an ``orc_params`` built from a scene and keeps the arrays it points at alive."""
 
-    def __init__(self, scene):
+    def __init__(self, scene, dtype: str = "f64"):
+        """dtype "f32": the single-precision build of the same source (8(f) f1, Table B.1 of the paper)."""
         self.scene = scene
-        p = OrcParams()
+        self.T = T = types(dtype)
+        p = T.OrcParams()
         for name in ("a", "mks_h", "mks_r0", "mass", "r_cam", "incl_deg", "fov_M", "t_cam", "M_bh_g",
                      "D_src_cm", "M_unit_g", "step_c", "step_min", "step_max", "eps", "delta", "eps_polar",
                      "r_stop_in_factor", "r_stop_out_factor", "tau_cutoff", "tp_over_te", "gamma_ad",
@@ -110,10 +139,10 @@ class Oracle:
                      "n1", "n2", "n3", "nt", "grid_dtype", "slow_light", "snapshot", "te_model"):
             setattr(p, name, int(getattr(scene, name)))
         m = list(scene.model) + [0.0] * (16 - len(scene.model))
-        p.model = (C.c_double * 16)(*m[:16])
-        self._freq = np.ascontiguousarray(np.asarray(scene.freq_hz, dtype=np.float64))
+        p.model = (T.REAL * 16)(*m[:16])
+        self._freq = np.ascontiguousarray(np.asarray(scene.freq_hz, dtype=T.np_real))
         p.n_freq = int(self._freq.size)
-        p.freq_hz = self._freq.ctypes.data_as(C.POINTER(C.c_double))
+        p.freq_hz = self._freq.ctypes.data_as(C.POINTER(T.REAL))
         self._grid = None
         if getattr(scene, "grid", None) is not None:
             want = np.float32 if scene.grid_dtype == 1 else np.float64
@@ -122,7 +151,7 @@ class Oracle:
             assert self._grid.size == expect, (self._grid.shape, expect)
             p.grid = self._grid.ctypes.data
         self.p = p
-        self.lib = lib()
+        self.lib = T.lib
 
     # ---- geometry -------------------------------------------------------------------
     @property
@@ -130,102 +159,102 @@ class Oracle:
         return self.lib.orc_horizon(C.byref(self.p))
 
     def metric(self, X):
-        g = _D44()
-        self.lib.orc_metric_mks(C.byref(self.p), _D4(*X), g)
+        g = self.T.D44()
+        self.lib.orc_metric_mks(C.byref(self.p), self.T.D4(*X), g)
         return np.array(g)
 
     def metric_inv(self, X):
-        g = _D44()
-        self.lib.orc_metric_mks_inv(C.byref(self.p), _D4(*X), g)
+        g = self.T.D44()
+        self.lib.orc_metric_mks_inv(C.byref(self.p), self.T.D4(*X), g)
         return np.array(g)
 
     def dmetric(self, X):
-        dg = _D444()
-        self.lib.orc_dmetric_mks(C.byref(self.p), _D4(*X), dg)
+        dg = self.T.D444()
+        self.lib.orc_dmetric_mks(C.byref(self.p), self.T.D4(*X), dg)
         return np.array(dg)
 
     def christoffel(self, X):
-        G = _D444()
-        self.lib.orc_christoffel_mks(C.byref(self.p), _D4(*X), G)
+        G = self.T.D444()
+        self.lib.orc_christoffel_mks(C.byref(self.p), self.T.D4(*X), G)
         return np.array(G)
 
     def rhs(self, X, K):
-        f = _D4()
-        self.lib.orc_rhs(C.byref(self.p), _D4(*X), _D4(*K), f)
+        f = self.T.D4()
+        self.lib.orc_rhs(C.byref(self.p), self.T.D4(*X), self.T.D4(*K), f)
         return np.array(f)
 
     def null_norm(self, X, K) -> float:
-        return self.lib.orc_null_norm(C.byref(self.p), _D4(*X), _D4(*K))
+        return self.lib.orc_null_norm(C.byref(self.p), self.T.D4(*X), self.T.D4(*K))
 
     def conserved(self, X, K):
-        E, L, Q = C.c_double(), C.c_double(), C.c_double()
-        self.lib.orc_conserved(C.byref(self.p), _D4(*X), _D4(*K), C.byref(E), C.byref(L), C.byref(Q))
+        E, L, Q = self.T.REAL(), self.T.REAL(), self.T.REAL()
+        self.lib.orc_conserved(C.byref(self.p), self.T.D4(*X), self.T.D4(*K), C.byref(E), C.byref(L), C.byref(Q))
         return E.value, L.value, Q.value
 
     def camera(self, alpha, beta):
-        X, K = _D4(), _D4()
+        X, K = self.T.D4(), self.T.D4()
         self.lib.orc_camera_ab(C.byref(self.p), float(alpha), float(beta), X, K)
         return np.array(X), np.array(K)
 
     def pixel_ab(self, ix, iy):
-        al, be = C.c_double(), C.c_double()
+        al, be = self.T.REAL(), self.T.REAL()
         self.lib.orc_pixel_ab(C.byref(self.p), int(ix), int(iy), C.byref(al), C.byref(be))
         return al.value, be.value
 
     def step_size(self, X, K) -> float:
-        return self.lib.orc_step_size(C.byref(self.p), _D4(*X), _D4(*K))
+        return self.lib.orc_step_size(C.byref(self.p), self.T.D4(*X), self.T.D4(*K))
 
     def rk4_step(self, X, K, dl):
-        Xc, Kc = _D4(*X), _D4(*K)
+        Xc, Kc = self.T.D4(*X), self.T.D4(*K)
         self.lib.orc_rk4_step(C.byref(self.p), Xc, Kc, float(dl))
         return np.array(Xc), np.array(Kc)
 
     def verlet_step(self, X, K, dl, corrector=False):
-        Xc, Kc = _D4(*X), _D4(*K)
+        Xc, Kc = self.T.D4(*X), self.T.D4(*K)
         self.lib.orc_verlet_step(C.byref(self.p), Xc, Kc, float(dl), 1 if corrector else 0)
         return np.array(Xc), np.array(Kc)
 
     def rk2_step(self, X, K, dl):
-        Xc, Kc = _D4(*X), _D4(*K)
+        Xc, Kc = self.T.D4(*X), self.T.D4(*K)
         self.lib.orc_rk2_step(C.byref(self.p), Xc, Kc, float(dl))
         return np.array(Xc), np.array(Kc)
 
     def step(self, X, K, dl):
         """One step of the scene's integrator (0 RK4, 1 Verlet, 2 Verlet + corrector, 3 RK2)."""
-        Xc, Kc = _D4(*X), _D4(*K)
+        Xc, Kc = self.T.D4(*X), self.T.D4(*K)
         self.lib.orc_step(C.byref(self.p), Xc, Kc, float(dl))
         return np.array(Xc), np.array(Kc)
 
     # ---- plasma + transfer ----------------------------------------------------------
     def grid_interp(self, X):
-        prim = (C.c_double * 8)()
-        ok = self.lib.orc_grid_interp(C.byref(self.p), _D4(*X), prim)
+        prim = (self.T.REAL * 8)()
+        ok = self.lib.orc_grid_interp(C.byref(self.p), self.T.D4(*X), prim)
         return (np.array(prim) if ok else None)
 
     def plasma(self, X):
-        ne, th, B, sf = C.c_double(), C.c_double(), C.c_double(), C.c_double()
-        u, p = _D4(), _D4()
-        ok = self.lib.orc_plasma(C.byref(self.p), _D4(*X), C.byref(ne), C.byref(th), C.byref(B), u, p, C.byref(sf))
+        ne, th, B, sf = self.T.REAL(), self.T.REAL(), self.T.REAL(), self.T.REAL()
+        u, p = self.T.D4(), self.T.D4()
+        ok = self.lib.orc_plasma(C.byref(self.p), self.T.D4(*X), C.byref(ne), C.byref(th), C.byref(B), u, p, C.byref(sf))
         if not ok:
             return None
         return dict(n_e=ne.value, theta_e=th.value, B=B.value, u=np.array(u), p=np.array(p), sin_fixed=sf.value)
 
     def transfer(self, X, K, h, I, tau):
-        I = np.ascontiguousarray(I, dtype=np.float64).copy()
-        tau = np.ascontiguousarray(tau, dtype=np.float64).copy()
-        ok = self.lib.orc_transfer(C.byref(self.p), _D4(*X), _D4(*K), C.c_double(h),
+        I = np.ascontiguousarray(I, dtype=self.T.np_real).copy()
+        tau = np.ascontiguousarray(tau, dtype=self.T.np_real).copy()
+        ok = self.lib.orc_transfer(C.byref(self.p), self.T.D4(*X), self.T.D4(*K), self.T.REAL(h),
                                    I.ctypes.data_as(C.c_void_p), tau.ctypes.data_as(C.c_void_p))
         return ok, I, tau
 
     # ---- rays and images ------------------------------------------------------------
     def trace(self, alpha, beta, record_path: bool = False, monitor_null: bool = False, max_path: int = 400000):
         nf = self.p.n_freq
-        I = np.zeros(nf)
-        tau = np.zeros(nf)
-        res = RayResult()
+        I = np.zeros(nf, dtype=self.T.np_real)
+        tau = np.zeros(nf, dtype=self.T.np_real)
+        res = self.T.RayResult()
         path = None
         if record_path:
-            path = np.zeros((max_path, 8))
+            path = np.zeros((max_path, 8), dtype=self.T.np_real)
         self.lib.orc_trace_ray(C.byref(self.p), float(alpha), float(beta), I.ctypes.data, tau.ctypes.data,
                                C.byref(res), path.ctypes.data if path is not None else None,
                                max_path if path is not None else 0, 1 if monitor_null else 0)
@@ -238,8 +267,8 @@ class Oracle:
     def render_disk(self):
         """Thin-disk workload: dict(image = sum of g^p/r^2 over counted crossings, redshift = g of the first one)."""
         p = self.p
-        image = np.zeros((1, p.ny, p.nx))
-        red = np.zeros((1, p.ny, p.nx))
+        image = np.zeros((1, p.ny, p.nx), dtype=self.T.np_real)
+        red = np.zeros((1, p.ny, p.nx), dtype=self.T.np_real)
         status = np.zeros((p.ny, p.nx), dtype=np.int32)
         nsteps = np.zeros((p.ny, p.nx), dtype=np.int32)
         steps, sampled = C.c_uint64(), C.c_uint64()
@@ -249,9 +278,9 @@ class Oracle:
         return dict(image=image, redshift=red, status=status, nsteps=nsteps, steps=steps.value, sampled=sampled.value)
 
     def line_profile(self, image_I, image_g, nbins, g_min, g_max):
-        a = np.ascontiguousarray(image_I, dtype=np.float64)
-        b = np.ascontiguousarray(image_g, dtype=np.float64)
-        hist = np.zeros(int(nbins))
+        a = np.ascontiguousarray(image_I, dtype=self.T.np_real)
+        b = np.ascontiguousarray(image_g, dtype=self.T.np_real)
+        hist = np.zeros(int(nbins), dtype=self.T.np_real)
         self.lib.orc_line_profile(C.byref(self.p), a.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p), int(nbins),
                                   float(g_min), float(g_max), hist.ctypes.data_as(C.c_void_p))
         return hist
@@ -259,7 +288,7 @@ class Oracle:
     def render(self, rows=None, row_stride: int = 1):
         """Full image (or rows [row0,row1) with a stride).  Returns dict(image, status, nsteps, steps, sampled)."""
         p = self.p
-        image = np.zeros((p.n_freq, p.ny, p.nx))
+        image = np.zeros((p.n_freq, p.ny, p.nx), dtype=self.T.np_real)
         status = np.zeros((p.ny, p.nx), dtype=np.int32)
         nsteps = np.zeros((p.ny, p.nx), dtype=np.int32)
         steps, sampled = C.c_uint64(), C.c_uint64()
@@ -270,54 +299,59 @@ class Oracle:
         return dict(image=image, status=status, nsteps=nsteps, steps=steps.value, sampled=sampled.value)
 
     def flux(self, image):
-        image = np.ascontiguousarray(image, dtype=np.float64)
-        out = np.zeros(self.p.n_freq)
+        image = np.ascontiguousarray(image, dtype=self.T.np_real)
+        out = np.zeros(self.p.n_freq, dtype=self.T.np_real)
         self.lib.orc_flux(C.byref(self.p), image.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p))
         return out
 
 
 # free functions -----------------------------------------------------------------------
-def planck(nu, theta_e):
-    return lib().orc_planck(float(nu), float(theta_e))
+def planck(nu, theta_e, dtype="f64"):
+    return lib(dtype).orc_planck(float(nu), float(theta_e))
 
 
-def emissivity(nu, n_e, theta_e, B, sin_th, k2_mode=0):
-    return lib().orc_emissivity(float(nu), float(n_e), float(theta_e), float(B), float(sin_th), int(k2_mode))
+def emissivity(nu, n_e, theta_e, B, sin_th, k2_mode=0, dtype="f64"):
+    return lib(dtype).orc_emissivity(float(nu), float(n_e), float(theta_e), float(B), float(sin_th), int(k2_mode))
 
 
-def r_isco(a):
-    return lib().orc_r_isco(float(a))
+def r_isco(a, dtype="f64"):
+    return lib(dtype).orc_r_isco(float(a))
 
 
-def bessel_k2(x):
-    return lib().orc_bessel_k2(float(x))
+def bessel_k2(x, dtype="f64"):
+    return lib(dtype).orc_bessel_k2(float(x))
 
 
-def transfer_update(I, tau, j, alpha, nu_hat, Lcm, h):
-    Ic, tc = C.c_double(I), C.c_double(tau)
-    lib().orc_transfer_update(C.byref(Ic), C.byref(tc), j, alpha, nu_hat, Lcm, h)
+def transfer_update(I, tau, j, alpha, nu_hat, Lcm, h, dtype="f64"):
+    T = types(dtype)
+    Ic, tc = T.REAL(I), T.REAL(tau)
+    T.lib.orc_transfer_update(C.byref(Ic), C.byref(tc), j, alpha, nu_hat, Lcm, h)
     return Ic.value, tc.value
 
 
-def mks_theta(h, x2):
-    th, d1, d2 = C.c_double(), C.c_double(), C.c_double()
-    lib().orc_mks_theta(float(h), float(x2), C.byref(th), C.byref(d1), C.byref(d2))
+def mks_theta(h, x2, dtype="f64"):
+    T = types(dtype)
+    th, d1, d2 = T.REAL(), T.REAL(), T.REAL()
+    T.lib.orc_mks_theta(float(h), float(x2), C.byref(th), C.byref(d1), C.byref(d2))
     return th.value, d1.value, d2.value
 
 
-def x2_of_theta(h, theta, tol=1e-15):
-    x2 = C.c_double()
-    it = lib().orc_x2_of_theta(float(h), float(theta), float(tol), C.byref(x2))
+def x2_of_theta(h, theta, tol=1e-15, dtype="f64"):
+    T = types(dtype)
+    x2 = T.REAL()
+    it = T.lib.orc_x2_of_theta(float(h), float(theta), float(tol), C.byref(x2))
     return x2.value, it
 
 
-def metric_ks(a, m, r, th):
-    g = _D44()
-    lib().orc_metric_ks(float(a), float(m), float(r), float(th), g)
+def metric_ks(a, m, r, th, dtype="f64"):
+    T = types(dtype)
+    g = T.D44()
+    T.lib.orc_metric_ks(float(a), float(m), float(r), float(th), g)
     return np.array(g)
 
 
-def metric_ks_inv(a, m, r, th):
-    g = _D44()
-    lib().orc_metric_ks_inv(float(a), float(m), float(r), float(th), g)
+def metric_ks_inv(a, m, r, th, dtype="f64"):
+    T = types(dtype)
+    g = T.D44()
+    T.lib.orc_metric_ks_inv(float(a), float(m), float(r), float(th), g)
     return np.array(g)

@@ -822,16 +822,17 @@ int orc_render(const orc_params *P, real *image, int32_t *status, int32_t *nstep
 /* O8: F_k [Jy] = 1e23 * sum_pix I_k * (fov/nx)(fov/ny) L^2 / D^2, Kahan-compensated, row-major order */
 void orc_flux(const orc_params *P, const real *image, real *flux_jy)
 {
-    real Lcm = ORC_G * P->M_bh_g / (ORC_C * ORC_C);
-    real scale = 1e23 * (P->fov_M / P->nx) * (P->fov_M / P->ny) * Lcm * Lcm / (P->D_src_cm * P->D_src_cm);
+    /* the sum and the scale factor are double in every build: D^2 ~ 7e44 cm^2 is beyond the range of a float */
+    double Lcm = ORC_G * P->M_bh_g / (ORC_C * ORC_C);
+    double scale = 1e23 * ((double)P->fov_M / P->nx) * ((double)P->fov_M / P->ny) * Lcm * Lcm / (P->D_src_cm * P->D_src_cm);
     size_t npix = (size_t)P->nx * P->ny;
     for (int k = 0; k < P->n_freq; ++k) {
-        real s = 0.0, c = 0.0;
+        double s = 0.0, c = 0.0;
         for (size_t i = 0; i < npix; ++i) {
-            real y = image[(size_t)k * npix + i] - c, t = s + y;
+            double y = (double)image[(size_t)k * npix + i] - c, t = s + y;
             c = (t - s) - y; s = t;
         }
-        flux_jy[k] = s * scale;
+        flux_jy[k] = (real)(s * scale);
     }
 }
 

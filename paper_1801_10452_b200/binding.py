@@ -14,7 +14,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libraptor_b200.so")
-ABI_VERSION = 1
+ABI_VERSION = 2
 MAX_FREQ = 64
 
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
@@ -24,7 +24,7 @@ STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 
 SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_render_disk",
            "raptor_line_profile", "raptor_set_camera_time", "raptor_set_window", "raptor_upload_snapshot",
            "raptor_light_curve", "raptor_spectrum", "raptor_flux",
-           "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_null_norm", "raptor_set_null_monitor", "raptor_get_counters", "raptor_fp64_peak",
+           "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_null_norm", "raptor_set_null_monitor", "raptor_get_counters", "raptor_fp64_peak", "raptor_fp64_probe",
            "raptor_destroy", "raptor_last_error")
 
 
@@ -45,6 +45,7 @@ class RaptorParams(C.Structure):
         ("max_steps", C.c_int32), ("n_freq", C.c_int32), ("plasma_model", C.c_int32), ("k2_mode", C.c_int32),
         ("n1", C.c_int32), ("n2", C.c_int32), ("n3", C.c_int32), ("nt", C.c_int32),
         ("grid_dtype", C.c_int32), ("slow_light", C.c_int32), ("snapshot", C.c_int32), ("te_model", C.c_int32),
+        ("precision", C.c_int32), ("reserved_", C.c_int32),
     ]
 
 
@@ -85,6 +86,7 @@ def lib():
         L.raptor_set_null_monitor.argtypes = [vp, vp]
         L.raptor_get_counters.argtypes = [vp, u64p, u64p, u64p]
         L.raptor_fp64_peak.argtypes = [i32, dp, dp]
+        L.raptor_fp64_probe.argtypes = [i32, i32, dp, dp]
         L.raptor_destroy.argtypes = [vp]
         L.raptor_last_error.argtypes = [vp]
         L.raptor_last_error.restype = C.c_char_p
@@ -112,6 +114,7 @@ def params_from_scene(scene):
     for name in ("nx", "ny", "integrator", "step_policy", "max_steps", "plasma_model", "k2_mode",
                  "n1", "n2", "n3", "nt", "grid_dtype", "slow_light", "snapshot", "te_model"):
         setattr(p, name, int(getattr(scene, name)))
+    p.precision = int(getattr(scene, "precision", 0))
     m = list(scene.model) + [0.0] * 16
     p.model = (C.c_double * 16)(*m[:16])
     freq = np.ascontiguousarray(np.asarray(scene.freq_hz, dtype=np.float64))
@@ -212,6 +215,13 @@ def raptor_fp64_peak(iters: int = 1 << 16):
     tf, ms = C.c_double(), C.c_double()
     _check(lib().raptor_fp64_peak(int(iters), C.byref(tf), C.byref(ms)))
     return tf.value, ms.value
+
+
+def raptor_fp64_probe(form: int, iters: int = 1 << 13):
+    """(warp instructions per second over the device, nominal SM clock in Hz) for operand form 0..4 (raptor.h)."""
+    rate, clk = C.c_double(), C.c_double()
+    _check(lib().raptor_fp64_probe(int(form), int(iters), C.byref(rate), C.byref(clk)))
+    return rate.value, clk.value
 
 
 # ---- convenience wrapper ----------------------------------------------------------------------

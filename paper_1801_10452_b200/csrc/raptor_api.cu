@@ -26,6 +26,7 @@ struct raptor_ctx {
     void* d_grid = nullptr;
     size_t grid_bytes = 0;
     double* d_freq = nullptr;
+    double nu0 = 0.0;                      // first frequency (precision = 1 has exactly one)
     unsigned int* d_queue = nullptr;
     unsigned long long* d_counters = nullptr;
     double* d_partial = nullptr;      // flux partial sums [n_freq][chunks]
@@ -37,6 +38,8 @@ struct raptor_ctx {
     double* d_scratch_flux = nullptr;
     size_t scratch_pixels = 0;
     cudaStream_t own_stream = nullptr;
+    KPf kpf;                               // precision = 1
+    float* d_grid_f32 = nullptr;           // precision = 1: (float) of d_grid
     double* d_null_max = nullptr;          // raptor_set_null_monitor: caller-owned output of the next render / trace calls
     cudaEvent_t ev_last = nullptr;         // recorded after every asynchronous call: raptor_render_host orders itself after it
     char err[512] = {0};
@@ -116,6 +119,11 @@ static int validate(const raptor_params* p) {
         if (!(p->model[1] > 0.0) || !(p->model[2] >= 1.0) || !std::isfinite(p->model[3]))
             return fail(nullptr, RAPTOR_EINVAL, "DISK: model = [r_in (<= 0: ISCO), r_out > 0, max_order >= 1, p]");
     }
+    if (p->precision != 0 && p->precision != 1) return fail(nullptr, RAPTOR_EINVAL, "precision %d: 0 (FP64) or 1 (FP32)", p->precision);
+    if (p->precision == 1 && !(p->plasma_model == RAPTOR_GRID2D && p->integrator == 3 && p->step_policy == 1 && p->n_freq == 1 &&
+                               p->k2_mode == 0 && p->te_model == 0))
+        return fail(nullptr, RAPTOR_EUNSUPPORTED, "precision 1 (FP32) is built for the paper's performance configuration only: "
+                                                  "GRID2D, integrator 3 (RK2), step_policy 1, n_freq 1, k2_mode 0, te_model 0");
     if (p->k2_mode != 0 && p->k2_mode != 1) return fail(nullptr, RAPTOR_EINVAL, "k2_mode %d: 0 (K2 = 2 Theta^2, PAPER.md:303) or 1 (exact K2)", p->k2_mode);
     if (p->te_model != 0 && p->te_model != 1) return fail(nullptr, RAPTOR_EINVAL, "te_model %d: 0 (constant T_p/T_e) or 1 (Eq. 47)", p->te_model);
     if (p->te_model == 1 && !(p->model[0] >= 0.0 && p->model[1] >= 0.0)) return fail(nullptr, RAPTOR_EINVAL, "te_model 1 needs model[0] = R_low >= 0, model[1] = R_high >= 0");
@@ -185,6 +193,21 @@ static void build_kp(raptor_ctx* c) {
     k.slow_light = p.slow_light; k.snapshot = p.snapshot;
 }
 
+// float copies of the kernel parameters (precision = 1); every value is computed in double and rounded once
+static void build_kpf(raptor_ctx* c) {
+    const KP& k = c->kp;
+    KPf& f = c->kpf;
+    std::memset(&f, 0, sizeof(f));
+    f.a = (float)k.a; f.a2 = (float)k.a2; f.twoa = (float)k.twoa; f.m = (float)k.m; f.twom = (float)k.twom; f.omh = (float)k.omh; f.r0 = (float)k.r0;
+    f.r_cam = (float)k.r_cam; f.sin_i = (float)k.sin_i; f.cos_i = (float)k.cos_i; f.sq1mc2 = (float)k.sq1mc2;
+    f.x1_cam = (float)k.x1_cam; f.x2_cam = (float)k.x2_cam; f.dth_cam = (float)k.dth_cam; f.t_cam = (float)k.t_cam; f.fov = (float)k.fov;
+    f.eps = (float)k.eps; f.delta = (float)k.delta; f.r_in = (float)k.r_in; f.r_out = (float)k.r_out; f.tau_cutoff = (float)k.tau_cutoff;
+    f.Lcm = (float)k.Lcm; f.ne_scale = (float)k.ne_scale; f.B0 = (float)k.B0; f.thetae_scale = (float)k.thetae_scale;
+    f.x1_first = (float)k.x1_first; f.inv_d1 = (float)k.inv_d1; f.nu_obs = (float)c->nu0;
+    f.grid = c->d_grid_f32;
+    f.nx = k.nx; f.ny = k.ny; f.max_steps = k.max_steps; f.n1 = k.n1; f.n2 = k.n2; f.use_tau_cutoff = k.use_tau_cutoff;
+}
+
 extern "C" int raptor_create(const raptor_params* p, raptor_ctx** out) {
     if (!out) return fail(nullptr, RAPTOR_EINVAL, "out is NULL");
     *out = nullptr;
@@ -211,6 +234,7 @@ extern "C" int raptor_create(const raptor_params* p, raptor_ctx** out) {
         double tab[3 * RAPTOR_MAX_FREQ];
         for (int k = 0; k < p->n_freq; ++k) {
             const double nu = p->freq_hz[k];
+            if (k == 0) c->nu0 = nu;
             tab[k] = nu;
             tab[p->n_freq + k] = std::cbrt(std::sqrt(nu));
             tab[2 * p->n_freq + k] = (kC * kC) / (2.0 * kHPL * nu * nu * nu);
@@ -228,11 +252,18 @@ extern "C" int raptor_create(const raptor_params* p, raptor_ctx** out) {
         c->grid_bytes = (size_t)p->grid_bytes;
         CKC(cudaMalloc(&c->d_grid, c->grid_bytes));
         CKC(cudaMemcpy(c->d_grid, p->grid_host, c->grid_bytes, cudaMemcpyHostToDevice));
+        if (p->precision == 1) {
+            const size_t n = c->grid_bytes / sizeof(double);
+            CKC(cudaMalloc(&c->d_grid_f32, n * sizeof(float)));
+            CKC(launch_grid_to_f32((const double*)c->d_grid, c->d_grid_f32, n, 0));
+            CKC(cudaDeviceSynchronize());
+        }
     }
 #undef CKC
     c->p.freq_hz = nullptr;      // the context owns device copies only
     c->p.grid_host = nullptr;
     build_kp(c);
+    if (p->precision == 1) build_kpf(c);
     *out = c;
     return RAPTOR_OK;
 }
@@ -242,6 +273,8 @@ extern "C" int raptor_upload_grid(raptor_ctx* ctx, const void* grid_host, uint64
     if (!ctx->d_grid) return fail(ctx, RAPTOR_EINVAL, "context has no grid");
     if (!grid_host || grid_bytes != ctx->grid_bytes) return fail(ctx, RAPTOR_EINVAL, "grid_bytes %llu != %zu", (unsigned long long)grid_bytes, ctx->grid_bytes);
     CK(ctx, cudaMemcpyAsync(ctx->d_grid, grid_host, ctx->grid_bytes, cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream));
+    if (ctx->d_grid_f32)
+        CK(ctx, launch_grid_to_f32((const double*)ctx->d_grid, ctx->d_grid_f32, ctx->grid_bytes / sizeof(double), (cudaStream_t)cuda_stream));
     return mark(ctx, (cudaStream_t)cuda_stream);
 }
 
@@ -259,7 +292,13 @@ static int run_rays(raptor_ctx* ctx, RenderOut& O, cudaStream_t s) {
     if (O.frames <= 1) O.null_max = ctx->d_null_max;
     if (O.tile_stride == 0) { O.tile_offset = 0; O.tile_stride = 1; }
     CK(ctx, cudaMemsetAsync(ctx->d_queue, 0, sizeof(unsigned int), s));
-    CK(ctx, launch_render(ctx->kp, ctx->p.plasma_model, O, ctx->sm_count, s));
+    if (ctx->p.precision == 1) {
+        if (O.frames > 1 || O.null_max) return fail(ctx, RAPTOR_EUNSUPPORTED, "precision 1 (FP32): no light curves, no null monitor");
+        ctx->kpf.t_cam = (float)ctx->kp.t_cam;
+        CK(ctx, launch_render_f32(ctx->kpf, O, ctx->sm_count, s));
+    } else {
+        CK(ctx, launch_render(ctx->kp, ctx->p.plasma_model, O, ctx->sm_count, s));
+    }
     return mark(ctx, s);
 }
 
@@ -546,9 +585,39 @@ extern "C" int raptor_fp64_peak(int32_t iters, double* tflops, double* ms) {
     return RAPTOR_OK;
 }
 
+extern "C" int raptor_fp64_probe(int32_t form, int32_t iters, double* warp_inst_per_sec, double* sm_clock_hz) {
+    if (form < 0 || form > 4 || iters < 1 || !warp_inst_per_sec) return fail(nullptr, RAPTOR_EINVAL, "form 0..4, iters >= 1, output not NULL");
+    int dev = 0, sms = 0, khz = 0;
+    CK(nullptr, cudaGetDevice(&dev));
+    CK(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(nullptr, cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
+    double* d_out = nullptr;
+    CK(nullptr, cudaMalloc(&d_out, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CK(nullptr, cudaEventCreate(&e0));
+    CK(nullptr, cudaEventCreate(&e1));
+    const int blocks = sms * 4;                                     // 4 x 256 threads: 8 warps per sub-partition
+    float best = 1e30f;
+    cudaError_t err = cudaSuccess;
+    for (int rep = 0; rep < 4 && err == cudaSuccess; ++rep) {       // rep 0 warms up
+        cudaEventRecord(e0, 0);
+        err = launch_fp64_form(form, iters, blocks, d_out, 0);
+        cudaEventRecord(e1, 0);
+        if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+        float t = 0.f;
+        cudaEventElapsedTime(&t, e0, e1);
+        if (rep > 0 && t < best) best = t;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+    if (err != cudaSuccess) return fail(nullptr, RAPTOR_ECUDA, "fp64 form probe: %s", cudaGetErrorString(err));
+    *warp_inst_per_sec = 8.0 * (double)iters * 8.0 * (double)blocks / (best * 1e-3);     // 8 chains x 8 warps per CTA
+    if (sm_clock_hz) *sm_clock_hz = 1e3 * (double)khz;
+    return RAPTOR_OK;
+}
+
 extern "C" int raptor_destroy(raptor_ctx* ctx) {
     if (!ctx) return RAPTOR_OK;
-    cudaFree(ctx->d_grid); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_counters);
+    cudaFree(ctx->d_grid); cudaFree(ctx->d_grid_f32); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_counters);
     cudaFree(ctx->d_partial); cudaFree(ctx->d_profile_partial); cudaFree(ctx->d_lc_partial); cudaFree(ctx->d_scratch_image); cudaFree(ctx->d_scratch_flux);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);

@@ -39,6 +39,19 @@ struct RenderOut {
     double t_cam0, dt_frame;        // camera time of frame f: t_cam0 + f dt_frame
 };
 
+// Kernel parameters of the single-precision kernel (raptor_render_f32.cu): float copies, computed on the host in
+// double and rounded once; only combinations inside the float range (8(f) f1, Table B.1 of the paper).
+struct KPf {
+    float a, a2, twoa, m, twom, omh, r0;
+    float r_cam, sin_i, cos_i, sq1mc2, x1_cam, x2_cam, dth_cam, t_cam, fov;
+    float eps, delta, r_in, r_out, tau_cutoff;
+    float Lcm, ne_scale, B0, thetae_scale, x1_first, inv_d1, nu_obs;
+    const float* grid;          // device, [n1][n2][8] float: (float) of the context's float64 grid
+    int nx, ny, max_steps, n1, n2, use_tau_cutoff;
+};
+cudaError_t launch_render_f32(const KPf& P, const RenderOut& O, int sm_count, cudaStream_t stream);
+cudaError_t launch_grid_to_f32(const double* d_src, float* d_dst, size_t n, cudaStream_t stream);
+
 // raptor_render.cu: one explicit instantiation per (plasma model, integrator), one translation unit each
 template <int MODEL, int INTEG>
 cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, int block, cudaStream_t s);
@@ -51,5 +64,6 @@ cudaError_t launch_profile(const double* d_image, const double* d_red, size_t np
 cudaError_t launch_null_norm(const KP& P, int n, const double* d_XK, double* d_out, double* d_elq, cudaStream_t stream);
 cudaError_t launch_eval_rhs(const KP& P, int n, const double* d_XK, double* d_f, cudaStream_t stream);
 cudaError_t launch_fp64_peak(int iters, int blocks, double* d_out, cudaStream_t stream);
+cudaError_t launch_fp64_form(int mode, int iters, int blocks, double* d_out, cudaStream_t stream);
 
 }  // namespace raptor

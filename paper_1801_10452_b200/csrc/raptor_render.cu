@@ -21,7 +21,7 @@ namespace raptor {
 #define RAPTOR_FASTPATH 0
 #endif
 #ifndef RAPTOR_REFRESH
-#define RAPTOR_REFRESH 15      // library exp / sincos at the base point every (RAPTOR_REFRESH + 1)-th step
+#define RAPTOR_REFRESH 63      // library exp / sincos at the base point every (RAPTOR_REFRESH + 1)-th step
 #endif
 
 // --------------------------------------------------------------------------------------------
@@ -147,9 +147,9 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             const double e1 = hh * f1, e2 = hh * f2;                               // stage-3 point minus stage-2 point
             {
                 const double d1 = hl * K[1], d2 = hl * K[2];
-                geom_shift<H1>(P, G, X[1] + d1, X[2] + d2, d1, d2, Gs);
+                geom_shift<H1>(P, G, X[1], X[2], d1, d2, Gs);
             }
-            const double x1s3 = fma(hl, k1, X[1]), x2s3 = fma(hl, k2, X[2]);       // stage-3 point (library fallback only)
+            const double x1s2 = fma(hl, K[1], X[1]), x2s2 = fma(hl, K[2], X[2]);   // stage-2 point (library fallback only)
             geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
             if (FULLX) { s0 = a0 + f0; s3 = a3 + f3; }
             s1 = a1 + f1; s2 = a2 + f2;
@@ -157,7 +157,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             const double g1 = hl * f1, g2 = hl * f2;                               // dl/2 f_2 (x1, x2): end-point offset below
             // stage 3 at X + dl/2 k_2, K + dl/2 f_2
             k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-            geom_shift<H1>(P, Gs, x1s3, x2s3, e1, e2, Gt);
+            geom_shift<H1>(P, Gs, x1s2, x2s2, e1, e2, Gt);
             geodesic_rhs(P, Gt, k0, k1, k2, k3, f0, f1, f2, f3);
             if (FULLX) { s0 += f0; s3 += f3; }
             s1 += f1; s2 += f2;
@@ -165,7 +165,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             // stage 4 at X + dl k_3, K + dl f_3
             {
                 const double d1 = dl * k1, d2 = dl * k2;
-                geom_shift<H1>(P, G, X[1] + d1, X[2] + d2, d1, d2, Gs);
+                geom_shift<H1>(P, G, X[1], X[2], d1, d2, Gs);
             }
             k0 = fma(dl, f0, K[0]); k1 = fma(dl, f1, K[1]); k2 = fma(dl, f2, K[2]); k3 = fma(dl, f3, K[3]);
             geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
@@ -182,7 +182,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             geodesic_rhs(P, G, K[0], K[1], K[2], K[3], f0, f1, f2, f3);
             k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
             const double d1 = hl * K[1], d2 = hl * K[2];
-            geom_shift<H1>(P, G, X[1] + d1, X[2] + d2, d1, d2, Gs);
+            geom_shift<H1>(P, G, X[1], X[2], d1, d2, Gs);
             geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
             // new point minus midpoint: dl k_mid - dl/2 K
             t1 = fma(dl, k1, -d1); t2 = fma(dl, k2, -d2);
@@ -199,7 +199,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             if (FULLX) { X[0] += fma(hd2, f0, dl * K[0]); X[3] += fma(hd2, f3, dl * K[3]); }
             X[1] += t1; X[2] += t2;
             p0 = fma(dl, f0, K[0]); p1 = fma(dl, f1, K[1]); p2 = fma(dl, f2, K[2]); p3 = fma(dl, f3, K[3]);   // Eq. 18
-            geom_shift<H1>(P, G, X[1], X[2], t1, t2, Gs);
+            geom_shift<H1, true>(P, G, X[1], X[2], t1, t2, Gs);
             geodesic_rhs(P, Gs, p0, p1, p2, p3, g0, g1, g2, g3);                                // Eq. 19
             p0 = fma(hl, f0 + g0, K[0]); p1 = fma(hl, f1 + g1, K[1]);                           // Eq. 20
             p2 = fma(hl, f2 + g2, K[2]); p3 = fma(hl, f3 + g3, K[3]);
@@ -222,7 +222,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         if ((n & RAPTOR_REFRESH) == 0) { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
         else if (have_G) { }
         else if (INTEG == I_VERLET || INTEG == I_VERLET_C) G = Gs;
-        else geom_shift<H1>(P, Gs, X[1], X[2], t1, t2, G);
+        else geom_shift<H1, true>(P, Gs, X[1], X[2], t1, t2, G);
         if (MON) {
             Met M;
             met_eval(P, G, M);

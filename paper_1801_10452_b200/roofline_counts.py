@@ -4,7 +4,9 @@ The counts are MEASURED, not typed in: one ncu pass per workload W over the same
 
     python bench.py --workload W --steps 1 --warmup 3 --no-cpu-baseline > gpurun_out/bench_W.json   (must exit 0) &&
     ncu --metrics smsp__sass_thread_inst_executed_op_dfma_pred_on.sum,smsp__sass_thread_inst_executed_op_dmul_pred_on.sum,\
-smsp__sass_thread_inst_executed_op_dadd_pred_on.sum,smsp__inst_executed_pipe_fp64.sum,smsp__inst_executed.sum,\
+smsp__sass_thread_inst_executed_op_dadd_pred_on.sum,smsp__sass_thread_inst_executed_op_ffma_pred_on.sum,\
+smsp__sass_thread_inst_executed_op_fmul_pred_on.sum,smsp__sass_thread_inst_executed_op_fadd_pred_on.sum,\
+smsp__inst_executed_pipe_fp64.sum,smsp__inst_executed.sum,\
 smsp__thread_inst_executed.sum,gpu__time_duration.sum,sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active,\
 dram__bytes_read.sum,dram__bytes_write.sum \
         --clock-control none -k regex:k_render -s 3 -c 1 --csv --log-file gpurun_out/flops_W.csv \

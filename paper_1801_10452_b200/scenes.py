@@ -85,6 +85,7 @@ class Scene:
     grid_dtype: int = F64
     slow_light: int = 0
     snapshot: int = 0           # fast light: which snapshot of a GRID3DT series is used
+    precision: int = 0          # 0 = FP64 (the contract); 1 = FP32 (the paper's performance configuration only, Table B.1)
     x1_min: float = 0.0
     x1_max: float = 0.0
     t0: float = 0.0
@@ -322,7 +323,12 @@ def thin_disk(a: float = 0.0, incl_deg: float = 60.0, nx: int = 256, r_out: floa
     return Scene(**base)
 
 
-CONFIGS = {"C0": config_C0, "C1": config_C1, "C2": config_C2, "C3": config_C3, "C4": config_C4, "PB1": config_PB1}
+def config_PB1_f32(nx: int = 512, n1: int = 256, n2: int = 256) -> Scene:
+    """PB1 in the paper's own precision (Table B.1: "Single precision: yes")."""
+    return replace(config_PB1(nx=nx, n1=n1, n2=n2), name="PB1F32", precision=1)
+
+
+CONFIGS = {"C0": config_C0, "C1": config_C1, "C2": config_C2, "C3": config_C3, "C4": config_C4, "PB1": config_PB1, "PB1F32": config_PB1_f32}
 
 
 def config(name: str, **kw) -> Scene:

@@ -1,0 +1,112 @@
+"""GPU parity of the single-precision kernel (Table B.1 of the paper: "Single
+precision: yes", "RK2", eps = 0.03) against the single-precision build of the oracle (the same source, real = float).
+
+Tolerance (derived from the arithmetic): both sides round every operation to 24 bits, in a
+different order (FMA contraction and CUDA's expf / sincosf on the GPU, none and glibc on the CPU); a ray takes ~700
+steps, each contributing ~1e-7 of relative round-off that the geodesic amplifies by up to ~1e2 near the hole, so pixels
+agree to ~1e-4 typically and ~1e-2 at worst outside the photon ring, where round-off decides the fate of the ray.
+Bar: median <= 3e-4, >= 99 % of the pixels outside a 0.15 M band <= 2e-2, flux <= 2e-3, step counts within +-2 on
+>= 95 %, status equal on >= 99 %.  The FP32-vs-FP64 difference (a result in itself) is reported beside it."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+from helpers import rel_err, ring_mask
+from paper_1801_10452_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def rb():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1801_10452_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import oracle
+    return oracle
+
+
+def gpu_render(rb, scene):
+    with rb.Raptor(scene) as R:
+        image, status, nsteps = R.render()
+        flux = R.flux(image)
+        torch.cuda.synchronize()
+        return dict(image=image.cpu().numpy(), status=status.cpu().numpy(), nsteps=nsteps.cpu().numpy(),
+                    flux=flux.cpu().numpy(), counters=R.counters())
+
+
+def compare(scene, g, ref, ref_flux, tag):
+    keep = ~ring_mask(scene, 0.15)
+    e = rel_err(g["image"], ref["image"].astype(np.float64))[0][keep]
+    dn = np.abs(g["nsteps"].astype(np.int64) - ref["nsteps"])[keep]
+    rep = dict(median=float(np.median(e)), p99=float(np.quantile(e, 0.99)), frac_2e2=float((e <= 2e-2).mean()), max=float(e.max()),
+               status_eq=float((g["status"][keep] == ref["status"][keep]).mean()), nsteps_eq=float((dn == 0).mean()),
+               nsteps_pm2=float((dn <= 2).mean()), flux_err=float(abs(g["flux"][0] - ref_flux) / ref_flux))
+    print(tag, rep)
+    return rep
+
+
+@pytest.mark.parametrize("nx", [40, 128])
+def test_f32_kernel_against_the_f32_oracle(rb, orc, nx):
+    s = scenes.config_PB1_f32(nx=nx)
+    g = gpu_render(rb, s)
+    o32 = orc.Oracle(s, dtype="f32")
+    ref = o32.render()
+    rep = compare(s, g, ref, float(o32.flux(ref["image"])[0]), f"PB1F32 {nx}^2 GPU f32 vs oracle f32:")
+    assert rep["median"] <= 3e-4 and rep["frac_2e2"] >= 0.99, rep
+    assert rep["flux_err"] <= 2e-3, rep
+    assert rep["status_eq"] >= 0.99 and rep["nsteps_pm2"] >= 0.95, rep
+    assert np.isfinite(g["image"]).all() and (g["image"] >= 0).all()
+    assert g["counters"][0] == int(g["nsteps"].sum()) and g["counters"][2] == nx * nx
+    # the FP32-vs-FP64 difference: the same scene through the FP64 kernel
+    g64 = gpu_render(rb, replace(s, precision=0))
+    rep64 = compare(s, g, dict(image=g64["image"], nsteps=g64["nsteps"], status=g64["status"]), float(g64["flux"][0]),
+                    f"PB1F32 {nx}^2 GPU f32 vs GPU f64:")
+    assert rep64["median"] <= 1e-3 and rep64["flux_err"] <= 2e-3, rep64
+
+
+def test_f32_single_rays(rb, orc):
+    s = scenes.config_PB1_f32(nx=8)
+    rng = np.random.default_rng(32)
+    al, be = rng.uniform(-18, 18, 48), rng.uniform(-18, 18, 48)
+    with rb.Raptor(s) as R:
+        g = R.trace(al, be)
+    o = orc.Oracle(s, dtype="f32")
+    close = 0
+    for i in range(al.size):
+        r = o.trace(float(np.float32(al[i])), float(np.float32(be[i])))
+        if g["status"][i] != r["status"] or abs(int(g["nsteps"][i]) - r["nsteps"]) > 2:
+            continue                       # a ray whose fate round-off decided
+        close += 1
+        assert np.all(np.abs(g["XK"][i, 1:3] - r["X"][1:3]) <= 2e-3 * np.maximum(np.abs(r["X"][1:3]), 1.0)), (i, g["XK"][i], r["X"])
+        assert abs(g["I"][0, i] - r["I"][0]) <= 5e-2 * abs(r["I"][0]) + 1e-30
+    assert close >= 44
+
+
+def test_f32_is_refused_outside_the_papers_configuration(rb):
+    for bad in (dict(integrator=0), dict(step_policy=0), dict(freq_hz=(86e9, 230e9)), dict(k2_mode=1)):
+        with pytest.raises(rb.RaptorError) as ei:
+            rb.Raptor(replace(scenes.config_PB1_f32(nx=8), **bad))
+        assert ei.value.code == rb.EUNSUPPORTED
+    with pytest.raises(rb.RaptorError):
+        rb.Raptor(replace(scenes.config_C1(8), precision=1))
+    # light curves and the null monitor are FP64 only
+    s = scenes.config_PB1_f32(nx=8)
+    with rb.Raptor(s) as R:
+        buf = torch.zeros((64,), dtype=torch.float64, device="cuda")
+        rb.raptor_set_null_monitor(R.ctx, buf.data_ptr())
+        with pytest.raises(rb.RaptorError):
+            R.render()
+        rb.raptor_set_null_monitor(R.ctx, None)
+        with pytest.raises(rb.RaptorError):
+            R.light_curve(2, 0.0, 1.0)
+        R.render()
