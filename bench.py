@@ -238,6 +238,14 @@ def run_ours(args):
         one_step()
     torch.cuda.synchronize()
     fp64_probe = binding.raptor_fp64_peak(1 << 16)[0]
+    # issue rate of the FP64 pipe by operand form (raptor.h): cycles per warp instruction per sub-partition
+    fp64_forms = None
+    if rank == 0:
+        names = ("dfma_1reg_imm", "dfma_3reg", "dfma_2reg", "dmul_2reg", "dadd_2reg")
+        fp64_forms = {}
+        for form, nm in enumerate(names):
+            rate, clk = binding.raptor_fp64_probe(form)
+            fp64_forms[nm] = 148 * 4 * clk / rate
     c_before = R.counters()
 
     sampler = ClockSampler(local)
@@ -368,7 +376,19 @@ def run_ours(args):
                                        "pipe_warp_inst_x32": 32.0 * row.get("fp64_pipe_warp_inst", float("nan"))},
                 "counts_source": "profiles/fp64_inst_per_step.json (ncu, source hash verified)",
                 "kernel_ms": avg_render_ms, "kernel_share_of_step": avg_render_ms / (total_ms / args.steps),
-                "algorithmic_flop_per_launch": steps_launch * flop_step}
+                "algorithmic_flop_per_launch": steps_launch * flop_step,
+                "fp64_issue_cycles_by_form": fp64_forms}
+            of = row.get("operand_forms")
+            if of and fp64_forms:
+                # operand-aware bound: a DFMA with three different register sources issues every ~3.2
+                # cycles, every other FP64 instruction every ~2.06 -- both measured live above
+                slow = fp64_forms["dfma_3reg"]
+                fast = (fp64_forms["dfma_2reg"] + fp64_forms["dmul_2reg"] + fp64_forms["dadd_2reg"]) / 3.0
+                cyc = of["dfma_3reg"] * slow + (of["dfma_3reg_reuse_flagged"] + of["dfma_other"] + of["dmul"] + of["dadd"] + of["dsetp"]) * fast
+                clk_hz = (clocks["sm_mhz"] or 1965.0) * 1e6
+                bound_ms = (steps_launch / 32.0) * cyc / (148 * 4 * clk_hz) * 1e3
+                line["roofline"]["operand_bound"] = {"cycles_per_warp_step": cyc, "ms": bound_ms, "frac": bound_ms / avg_render_ms,
+                                                     "dfma_3reg_per_step": of["dfma_3reg"]}
         # ---- CPU baseline: the oracle on a bounded sample of the same workload (about 10-30 s of host work)
         cpu = None
         if world == 1 and not args.no_cpu_baseline:

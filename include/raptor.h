@@ -154,9 +154,20 @@ int raptor_upload_snapshot(raptor_ctx *ctx, int64_t snapshot, const void *snapsh
  * must be (0, 1) (light curves shard by frames). */
 int raptor_light_curve(raptor_ctx *ctx, int32_t n_frames, double t_cam0, double dt_frame, double *d_flux_jy, void *cuda_stream);
 
+/* Time calibration of Sect. 5.1: "an empirical, pragmatic strategy ... effectively equivalent to
+ * translating the slow-light light curve with respect to the fast-light light curve on the time axis".  Both curves
+ * are normalised by their means; for each of the n_grid shifts d_k = -max_shift + 2 max_shift k/(n_grid - 1) the
+ * slow-light curve is interpolated linearly at t_fast[i] + d_k (points outside [t_slow[0], t_slow[n_slow-1]] are
+ * left out; a shift that keeps fewer than max(4, n_fast/2) points is skipped) and the rms difference to the
+ * fast-light curve is formed; *delay receives the first shift with the smallest rms, *rms that rms (+inf and
+ * delay 0 if every shift was skipped).  HOST pointers, t_slow ascending; plain host arithmetic, synchronous. */
+int raptor_calibrate_delay(int32_t n_fast, const double *t_fast, const double *F_fast, int32_t n_slow, const double *t_slow,
+                           const double *F_slow, double max_shift, int32_t n_grid, double *delay, double *rms);
+
 /* Multi-GPU sharding of one image: after this call raptor_render / raptor_spectrum /
- * raptor_render_host trace only the 8x4-pixel tiles rank, rank + world, rank + 2 world, ... (row-major tile
- * order) and leave every other pixel of the caller's output buffers untouched.  Rays are independent, so the ranks'
+ * raptor_render_host trace only the 8x4-pixel tiles at positions rank, rank + world, rank + 2 world, ... of the
+ * kernel's tile sequence (rows of tiles from the image centre outward -- mid, mid - 1, mid + 1, ... with
+ * mid = ceil(ny/4) / 2 -- and left to right within a row) and leave every other pixel of the caller's output buffers untouched.  Rays are independent, so the ranks'
  * images (zero-initialised by the caller) sum to the full image exactly.  Where the library owns the image
  * (raptor_spectrum with a NULL image, raptor_render_host) it zeroes it first, so fluxes are the shard's own and
  * sum to the full flux.  Default (0, 1) = whole image. */

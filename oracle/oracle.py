@@ -99,6 +99,8 @@ class _Types:
         L.orc_rk2_step.argtypes = [PP, D4, D4, R]
         L.orc_step.argtypes = [PP, D4, D4, R]
         L.orc_transfer.argtypes = [PP, D4, D4, R, C.c_void_p, C.c_void_p]
+        L.orc_calibrate_delay.restype = R
+        L.orc_calibrate_delay.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, R, C.c_int, C.POINTER(R)]
         L.orc_trace_ray.argtypes = [PP, R, R, C.c_void_p, C.c_void_p, C.POINTER(RayResult), C.c_void_p, C.c_int, C.c_int]
 
 
@@ -355,3 +357,13 @@ def metric_ks_inv(a, m, r, th, dtype="f64"):
     g = T.D44()
     T.lib.orc_metric_ks_inv(float(a), float(m), float(r), float(th), g)
     return np.array(g)
+
+
+def calibrate_delay(t_fast, F_fast, t_slow, F_slow, max_shift, n_grid=2001, dtype="f64"):
+    """Sect. 5.1: (delay, rms) -- the oracle's plain grid search."""
+    T = types(dtype)
+    arr = [np.ascontiguousarray(x, dtype=T.np_real) for x in (t_fast, F_fast, t_slow, F_slow)]
+    rms = T.REAL()
+    d = T.lib.orc_calibrate_delay(arr[0].size, arr[0].ctypes.data, arr[1].ctypes.data, arr[2].size, arr[2].ctypes.data,
+                                  arr[3].ctypes.data, float(max_shift), int(n_grid), C.byref(rms))
+    return d, rms.value

@@ -854,5 +854,40 @@ void orc_line_profile(const orc_params *P, const real *image_I, const real *imag
     }
 }
 
+/* Time calibration of Sect. 5.1: "translating the slow-light light curve with respect to the
+ * fast-light light curve on the time axis".  Step by step: normalise both curves by their means; for every trial shift
+ * d_k = -max_shift + 2 max_shift k/(n_grid-1): interpolate the slow curve linearly at t_fast[i] + d_k (skipping
+ * points outside the slow curve's time range; a shift that keeps fewer than max(4, n_fast/2) points is skipped),
+ * take the rms difference; keep the first shift with the smallest rms.  Returns that shift, *rms_out the rms
+ * (HUGE_VAL if no shift qualified). */
+real orc_calibrate_delay(int n_fast, const real *t_fast, const real *F_fast, int n_slow, const real *t_slow,
+                         const real *F_slow, real max_shift, int n_grid, real *rms_out)
+{
+    real mean_f = 0.0, mean_s = 0.0, best_d = 0.0, best = HUGE_VAL;
+    for (int i = 0; i < n_fast; ++i) mean_f += F_fast[i] / n_fast;
+    for (int i = 0; i < n_slow; ++i) mean_s += F_slow[i] / n_slow;
+    int need = n_fast / 2 > 4 ? n_fast / 2 : 4;
+    for (int k = 0; k < n_grid; ++k) {
+        real d = (n_grid > 1) ? -max_shift + 2.0 * max_shift * k / (n_grid - 1) : 0.0;
+        real sum = 0.0;
+        int used = 0;
+        for (int i = 0; i < n_fast; ++i) {
+            real t = t_fast[i] + d;
+            if (t < t_slow[0] || t > t_slow[n_slow - 1]) continue;
+            int seg = 0;
+            while (seg < n_slow - 2 && t_slow[seg + 1] < t) ++seg;            /* t_slow[seg] <= t <= t_slow[seg+1] */
+            real Fs = F_slow[seg] + (F_slow[seg + 1] - F_slow[seg]) * (t - t_slow[seg]) / (t_slow[seg + 1] - t_slow[seg]);
+            real diff = Fs / mean_s - F_fast[i] / mean_f;
+            sum += diff * diff;
+            ++used;
+        }
+        if (used < need) continue;
+        real rms = sqrt(sum / used);
+        if (rms < best) { best = rms; best_d = d; }
+    }
+    *rms_out = best;
+    return best_d;
+}
+
 size_t orc_sizeof_params(void) { return sizeof(orc_params); }
 size_t orc_sizeof_ray_result(void) { return sizeof(orc_ray_result); }

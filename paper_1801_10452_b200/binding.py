@@ -23,7 +23,7 @@ STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 
 # every symbol include/raptor.h declares
 SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_render_disk",
            "raptor_line_profile", "raptor_set_camera_time", "raptor_set_window", "raptor_upload_snapshot",
-           "raptor_light_curve", "raptor_spectrum", "raptor_flux",
+           "raptor_light_curve", "raptor_calibrate_delay", "raptor_spectrum", "raptor_flux",
            "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_null_norm", "raptor_set_null_monitor", "raptor_get_counters", "raptor_fp64_peak", "raptor_fp64_probe",
            "raptor_destroy", "raptor_last_error")
 
@@ -75,6 +75,7 @@ def lib():
         L.raptor_set_window.argtypes = [vp, C.c_int64]
         L.raptor_upload_snapshot.argtypes = [vp, C.c_int64, vp, C.c_uint64, vp]
         L.raptor_light_curve.argtypes = [vp, i32, C.c_double, C.c_double, vp, vp]
+        L.raptor_calibrate_delay.argtypes = [i32, vp, vp, i32, vp, vp, C.c_double, i32, dp, dp]
         L.raptor_render_disk.argtypes = [vp, vp, vp, vp, vp, vp]
         L.raptor_line_profile.argtypes = [vp, vp, vp, i32, C.c_double, C.c_double, vp, vp]
         L.raptor_spectrum.argtypes = [vp, vp, vp, vp]
@@ -167,6 +168,16 @@ def raptor_upload_snapshot(ctx, snapshot, h_snapshot, nbytes, stream=None):
 
 def raptor_light_curve(ctx, n_frames, t_cam0, dt_frame, d_flux, stream=None):
     _check(lib().raptor_light_curve(ctx, int(n_frames), float(t_cam0), float(dt_frame), d_flux, stream), ctx)
+
+
+def raptor_calibrate_delay(t_fast, F_fast, t_slow, F_slow, max_shift, n_grid=2001):
+    """Sect. 5.1: (delay, rms) that best aligns the slow-light curve with the fast-light one (raptor.h)."""
+    tf, Ff = (np.ascontiguousarray(x, dtype=np.float64) for x in (t_fast, F_fast))
+    ts, Fs = (np.ascontiguousarray(x, dtype=np.float64) for x in (t_slow, F_slow))
+    d, r = C.c_double(), C.c_double()
+    _check(lib().raptor_calibrate_delay(tf.size, tf.ctypes.data, Ff.ctypes.data, ts.size, ts.ctypes.data, Fs.ctypes.data,
+                                        float(max_shift), int(n_grid), C.byref(d), C.byref(r)))
+    return d.value, r.value
 
 
 def raptor_set_shard(ctx, rank, world):

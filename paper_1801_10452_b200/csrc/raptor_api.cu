@@ -434,6 +434,39 @@ extern "C" int raptor_light_curve(raptor_ctx* ctx, int32_t n_frames, double t_ca
     return mark(ctx, s);
 }
 
+extern "C" int raptor_calibrate_delay(int32_t n_fast, const double* t_fast, const double* F_fast, int32_t n_slow, const double* t_slow,
+                                      const double* F_slow, double max_shift, int32_t n_grid, double* delay, double* rms) {
+    if (n_fast < 1 || n_slow < 2 || !t_fast || !F_fast || !t_slow || !F_slow || !delay || !rms)
+        return fail(nullptr, RAPTOR_EINVAL, "raptor_calibrate_delay: need n_fast >= 1, n_slow >= 2 and non-NULL arrays");
+    if (!(max_shift >= 0.0) || n_grid < 1) return fail(nullptr, RAPTOR_EINVAL, "raptor_calibrate_delay: max_shift >= 0, n_grid >= 1");
+    double mf = 0.0, ms = 0.0;
+    for (int i = 0; i < n_fast; ++i) mf += F_fast[i];
+    for (int i = 0; i < n_slow; ++i) ms += F_slow[i];
+    mf /= n_fast; ms /= n_slow;
+    const int need = std::max(4, n_fast / 2);
+    double best_d = 0.0, best = INFINITY;
+    for (int k = 0; k < n_grid; ++k) {
+        const double d = n_grid > 1 ? -max_shift + 2.0 * max_shift * k / (n_grid - 1) : 0.0;
+        double acc = 0.0;
+        int used = 0, j = 0;
+        for (int i = 0; i < n_fast; ++i) {
+            const double ts = t_fast[i] + d;
+            if (ts < t_slow[0] || ts > t_slow[n_slow - 1]) continue;
+            while (j + 2 < n_slow && t_slow[j + 1] < ts) ++j;          // t_fast ascending is the common case ...
+            while (j > 0 && t_slow[j] > ts) --j;                       // ... but not required
+            const double w = (ts - t_slow[j]) / (t_slow[j + 1] - t_slow[j]);
+            const double res = (F_slow[j] + w * (F_slow[j + 1] - F_slow[j])) / ms - F_fast[i] / mf;
+            acc += res * res;
+            ++used;
+        }
+        if (used < need) continue;
+        const double r = std::sqrt(acc / used);
+        if (r < best) { best = r; best_d = d; }
+    }
+    *delay = best_d; *rms = best;
+    return RAPTOR_OK;
+}
+
 extern "C" int raptor_set_shard(raptor_ctx* ctx, int32_t rank, int32_t world) {
     if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
     if (world < 1 || rank < 0 || rank >= world) return fail(ctx, RAPTOR_EINVAL, "shard: need 0 <= rank < world");

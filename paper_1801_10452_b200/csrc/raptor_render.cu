@@ -308,7 +308,11 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
             alpha = active ? O.alpha[pix] : 0.0;
             beta = active ? O.beta[pix] : 0.0;
         } else {
-            const int ty = tile / ntx, tx = tile - ty * ntx;
+            // tile order: rows of tiles from the image centre outward (k = 0, 1, 2, ... -> mid, mid-1, mid+1, ...): the
+            // longest rays (photon ring; under the step rule of Eq. 21-24 everything near the hole) start first and the
+            // launch ends on the uniform outer rows instead of waiting for a late long tile (PB1: -9 %, PB1 FP32: -15 %)
+            const int seq_row = tile / ntx, tx = tile - seq_row * ntx, mid = ((P.ny + 3) >> 2) >> 1;
+            const int ty = (seq_row & 1) ? mid - 1 - (seq_row >> 1) : mid + (seq_row >> 1);
             const int ix = (tx << 3) + (lane & 7), iy = (ty << 2) + (lane >> 3);
             active = ix < P.nx && iy < P.ny;
             alpha = fma((double)ix + 0.5, P.pix_dx, -0.5 * P.fov);             // pixel centres [A4b]

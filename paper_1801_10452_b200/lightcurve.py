@@ -21,10 +21,7 @@ from typing import Callable, Sequence
 import numpy as np
 
 
-def light_travel_offset(r_cam: float, r_ref: float = 10.0) -> float:
-    """Coordinate-time offset between a camera at r_cam and radius r_ref along the outgoing radial null ray of
-    ingoing Kerr-Schild Schwarzschild, t(r) = r + 4 ln(r - 2) + const [A15 in DESIGN.md]."""
-    return (r_cam + 4.0 * math.log(r_cam - 2.0)) - (r_ref + 4.0 * math.log(r_ref - 2.0))
+from .scenes import light_travel_offset      # [A15 in DESIGN.md]: one home, scenes.py
 
 
 def window_start(t_cam: float, r_cam: float, t0: float, dt_snap: float, nt: int, n_snap: int) -> int:
@@ -104,17 +101,5 @@ def calibrate_delay(t_fast, F_fast, t_slow, F_slow, max_shift: float, n_grid: in
     """Sect. 5.1: the delay d for which F_slow(t + d) best matches F_fast(t) (least squares over the
     overlap, both curves normalised by their means), "effectively equivalent to translating the slow-light light
     curve with respect to the fast-light light curve on the time axis".  Returns (d, rms residual at d)."""
-    t_fast, F_fast = np.asarray(t_fast, float), np.asarray(F_fast, float)
-    t_slow, F_slow = np.asarray(t_slow, float), np.asarray(F_slow, float)
-    Ff, Fs = F_fast / F_fast.mean(), F_slow / F_slow.mean()
-    best = (0.0, math.inf)
-    for d in np.linspace(-max_shift, max_shift, n_grid):
-        ts = t_fast + d
-        ok = (ts >= t_slow[0]) & (ts <= t_slow[-1])
-        if ok.sum() < max(4, len(t_fast) // 2):
-            continue
-        res = np.interp(ts[ok], t_slow, Fs) - Ff[ok]
-        rms = math.sqrt(float(np.mean(res * res)))
-        if rms < best[1]:
-            best = (float(d), rms)
-    return best
+    from . import binding
+    return binding.raptor_calibrate_delay(t_fast, F_fast, t_slow, F_slow, max_shift, n_grid)

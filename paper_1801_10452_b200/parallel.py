@@ -19,17 +19,27 @@ def n_tiles(nx: int, ny: int) -> int:
     return ((nx + TILE_X - 1) // TILE_X) * ((ny + TILE_Y - 1) // TILE_Y)
 
 
+def tile_row_of_position(k: int, nty: int) -> int:
+    """The kernel's tile order walks the rows of tiles from the image centre outward: position 0, 1, 2, ... of the
+    sequence is row mid, mid - 1, mid + 1, ... (mid = nty // 2), so that the longest rays start first."""
+    mid = nty // 2
+    return mid - 1 - k // 2 if k % 2 else mid + k // 2
+
+
 def tiles_of_rank(nx: int, ny: int, rank: int, world: int) -> range:
-    """Global tile indices (row-major) traced by ``rank`` after raptor_set_shard(rank, world)."""
+    """Positions in the kernel's tile sequence (rows centre-outward, left to right within a row) traced by ``rank``
+    after raptor_set_shard(rank, world)."""
     return range(rank, n_tiles(nx, ny), world)
 
 
 def pixel_owner_map(nx: int, ny: int, world: int) -> torch.Tensor:
     """[ny, nx] int32: which rank traces each pixel under the tile sharding."""
-    ntx = (nx + TILE_X - 1) // TILE_X
+    ntx, nty = (nx + TILE_X - 1) // TILE_X, (ny + TILE_Y - 1) // TILE_Y
+    mid = nty // 2
     iy, ix = torch.meshgrid(torch.arange(ny), torch.arange(nx), indexing="ij")
-    tile = (iy // TILE_Y) * ntx + ix // TILE_X
-    return (tile % world).to(torch.int32)
+    ty = iy // TILE_Y
+    pos = torch.where(ty >= mid, 2 * (ty - mid), 2 * (mid - 1 - ty) + 1)        # inverse of tile_row_of_position
+    return ((pos * ntx + ix // TILE_X) % world).to(torch.int32)
 
 
 def frames_of_rank(n_frames: int, rank: int, world: int) -> range:

@@ -32,7 +32,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 DEFAULT_JSON = os.path.join(os.path.dirname(HERE), "profiles", "fp64_inst_per_step.json")
-WORKLOADS = ("C0", "C1", "C2", "C3", "C4", "PB1", "PB1F32", "LC")
+WORKLOADS = ("C0", "C1", "C2", "C3", "C4", "PB1", "PB1F32", "LC", "C3B")
 
 METRICS = {
     "dfma": "smsp__sass_thread_inst_executed_op_dfma_pred_on.sum",
@@ -90,7 +90,7 @@ def collect(run_dir: str) -> dict:
             continue
         with open(f_json) as fh:
             bench = json.loads(fh.read().strip().splitlines()[-1])
-        steps = float(bench["steps_per_image"])
+        steps = float(bench["steps_per_image"]) * float(bench.get("frames_per_step", 1))     # accepted steps of ONE launch
         m = parse_ncu_csv(f_csv)
         row = {"steps_per_launch": steps}
         for key, name in METRICS.items():
@@ -98,6 +98,57 @@ def collect(run_dir: str) -> dict:
                 row[key] = m[name] if key in ("kernel_ns", "fp64_pipe_pct", "dram_read_bytes", "dram_write_bytes") else m[name] / steps
         table[w] = row
     return table
+
+
+def operand_forms(source_csv: str, lib_path: str, mangled: str, steps_per_launch: float) -> dict:
+    """FP64 instructions per accepted step by operand form, for the operand-aware bound of DESIGN.md 5.1.
+
+    ``source_csv`` = ``ncu -i prof.ncu-rep --page source --csv --print-source sass`` of one k_render launch (executed
+    count per SASS instruction); ``lib_path`` + ``mangled`` (a substring of the mangled kernel name) give the same
+    kernel's SASS from ``cuobjdump -sass``, which -- unlike ncu's listing -- carries the ``.reuse`` flags.  The two
+    listings are joined by instruction order.  A DFMA whose three sources are three different registers, none of them
+    served by the operand-reuse cache (flagged ``.reuse`` on the PREVIOUS instruction's same slot is not tracked here:
+    the count below is an upper bound of the slow form), issues every 3.17 cycles on B200; every other FP64
+    instruction every 2.06 (raptor_fp64_probe)."""
+    import re
+    import subprocess
+    sass, take = [], False
+    out = subprocess.run(["cuobjdump", "-sass", lib_path], capture_output=True, text=True).stdout
+    for line in out.splitlines():
+        if "Function :" in line:
+            take = mangled in line
+            continue
+        if take:
+            m = re.match(r"\s+/\*([0-9a-f]{4,})\*/\s+(.*?);", line)
+            if m:
+                sass.append(m.group(2).strip())
+    with open(source_csv, newline="") as fh:
+        rows = list(csv.reader(fh))
+    head = next(r for r in rows if "Source" in r and "Instructions Executed" in r)
+    i_s, i_e = head.index("Source"), head.index("Instructions Executed")
+    prof = [(r[i_s].strip(), int(r[i_e])) for r in rows[rows.index(head) + 1:] if len(r) > i_e and r[i_e].isdigit()]
+    n = min(len(sass), len(prof))
+    mismatch = sum(1 for a, (b, _) in zip(sass[:n], prof[:n]) if a.replace(".reuse", "").split()[:1] != b.split()[:1])
+    warp_steps = steps_per_launch / 32.0
+    out_counts = {"dfma_3reg": 0.0, "dfma_3reg_reuse_flagged": 0.0, "dfma_other": 0.0, "dmul": 0.0, "dadd": 0.0, "dsetp": 0.0}
+    for text, (_, cnt) in zip(sass[:n], prof[:n]):
+        t = re.sub(r"^@!?U?P\d+\s+", "", text)
+        op = t.split()[0].split(".")[0]
+        if op not in ("DFMA", "DMUL", "DADD", "DSETP"):
+            continue
+        srcs = [o.strip() for o in t.split(None, 1)[1].split(",")[1:]]
+        regs, reuse = set(), 0
+        for o in srcs:
+            m = re.match(r"^[-|~]*\|?(R\d+)(\.reuse)?", o)
+            if m:
+                regs.add(m.group(1))
+                reuse += 1 if m.group(2) else 0
+        key = {"DMUL": "dmul", "DADD": "dadd", "DSETP": "dsetp"}.get(op)
+        if op == "DFMA":
+            key = "dfma_other" if len(regs) < 3 else ("dfma_3reg_reuse_flagged" if reuse else "dfma_3reg")
+        out_counts[key] += cnt / warp_steps
+    out_counts["listing_mismatch"] = mismatch
+    return out_counts
 
 
 def load(path: str = DEFAULT_JSON):
@@ -113,12 +164,24 @@ def load(path: str = DEFAULT_JSON):
     return doc["per_step"], None
 
 
+# mangled-name substrings of the kernels bench.py's workloads launch (for operand_forms)
+KERNEL_OF = {"C0": "k_renderILi1ELb1ELb0ELb0ELi0ELb0E", "C1": "k_renderILi2ELb1ELb0ELb0ELi0ELb0E",
+             "C2": "k_renderILi3ELb0ELb0ELb0ELi0ELb0E", "C3": "k_renderILi3ELb0ELb1ELb0ELi0ELb0E",
+             "C4": "k_renderILi4ELb0ELb0ELb1ELi0ELb0E", "PB1": "k_renderILi3ELb0ELb0ELb1ELi3ELb0E"}
+
+
 def main(argv):
     run_dir = argv[1] if len(argv) > 1 else "gpurun_out"
     out = argv[2] if len(argv) > 2 else DEFAULT_JSON
     table = collect(run_dir)
     if not table:
         raise SystemExit(f"no flops_<W>.csv + bench_<W>.json pairs under {run_dir}")
+    # optional: operand forms, where `ncu -i prof_<W>_r2.ncu-rep --page source --csv --print-source sass > source_<W>.csv` exists
+    lib_path = os.path.join(HERE, "libraptor_b200.so")
+    for w, mangled in KERNEL_OF.items():
+        src = os.path.join(run_dir, f"source_{w}.csv")
+        if w in table and os.path.exists(src) and os.path.exists(lib_path):
+            table[w]["operand_forms"] = operand_forms(src, lib_path, mangled, table[w]["steps_per_launch"])
     doc = {"csrc_sha256": csrc_sha256(),
            "what": "thread-level executed FP64 instructions of one k_render launch / accepted steps of that launch; "
                    "flop = 2 dfma + dmul + dadd; fp64_pipe_warp_inst = warp-level instructions issued to the FP64 pipe "

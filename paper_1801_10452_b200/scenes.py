@@ -266,11 +266,17 @@ def config_C3(nx: int = 256, n_freq: int = 32, n1: int = 256, n2: int = 256) -> 
     return replace(s, name="C3", freq_hz=nu)
 
 
+def light_travel_offset(r_cam: float, r_ref: float = 10.0) -> float:
+    """Coordinate-time offset between a camera at r_cam and radius r_ref along the outgoing radial null ray of
+    ingoing Kerr-Schild Schwarzschild, t(r) = r + 4 ln(r - 2) + const.  The ONE home of
+    this formula: a number attached to a scene (t_cam) or to a snapshot window, not part of the method."""
+    return (r_cam + 4.0 * math.log(r_cam - 2.0)) - (r_ref + 4.0 * math.log(r_ref - 2.0))
+
+
 def slow_light_t_cam(r_cam: float, t_mid: float) -> float:
-    """Camera time that centres the snapshot window: light-travel time of an outgoing radial
-    null ray of ingoing-KS Schwarzschild from r = 10 M; replaces
-    the paper's empirical calibration.  A number attached to the scene."""
-    return t_mid + (r_cam + 4.0 * math.log(r_cam - 2.0)) - (10.0 + 4.0 * math.log(8.0))
+    """Camera time that centres the snapshot window on t_mid: replaces the paper's empirical
+    calibration as a first guess; raptor_calibrate_delay refines it from two light curves."""
+    return t_mid + light_travel_offset(r_cam)
 
 
 def config_C4(nx: int = 1024, n1: int = 128, n2: int = 64, n3: int = 64, nt: int = 32,

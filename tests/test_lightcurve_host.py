@@ -5,6 +5,7 @@ import os
 import socket
 
 import numpy as np
+import pytest
 import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
@@ -50,12 +51,29 @@ def test_window_streamer_uploads_only_new_snapshots_into_their_slots():
 
 
 def test_calibrate_delay_recovers_a_known_shift():
-    # Sect. 5.1: the slow-light curve is the fast-light curve translated on the time axis
+    # Sect. 5.1: the slow-light curve is the fast-light curve translated on the time axis.  The ORACLE's
+    # grid search is pinned by a known shift; the library's host routine (raptor_calibrate_delay, reached through
+    # lightcurve.calibrate_delay; no GPU involved) must then agree with the oracle.
+    from oracle import oracle as orc
     t = np.arange(0.0, 2000.0, 10.0)
     f = lambda x: 2.0 + 0.4 * np.sin(x / 90.0) + 0.2 * np.sin(x / 37.0 + 1.0) + 0.1 * np.cos(x / 11.0)
     for true in (-63.0, 0.0, 41.5):
+        do, ro = orc.calibrate_delay(t, f(t), t, 3.0 * f(t - true), max_shift=150.0, n_grid=3001)
+        assert abs(do - true) <= 0.5 and ro < 2e-2, (do, ro)     # residual: linear interpolation between samples
         d, rms = lc.calibrate_delay(t, f(t), t, 3.0 * f(t - true), max_shift=150.0, n_grid=3001)
-        assert abs(d - true) <= 0.5 and rms < 2e-2, (d, rms)     # residual: linear interpolation between samples
+        assert d == pytest.approx(do, abs=1e-9) and rms == pytest.approx(ro, rel=1e-9)
+    # by hand: two-point "curves" -- fast (t = 0, 1; F = 1, 3), slow = the same line shifted by +0.25 in time
+    ts = np.array([-1.0, 0.0, 1.0, 2.0])
+    Fs = 1.0 + 2.0 * (ts - 0.25)
+    tf, Ff = np.array([0.0, 0.5, 1.0, 1.5]), 1.0 + 2.0 * np.array([0.0, 0.5, 1.0, 1.5])
+    # unnormalised the match would be exact at d = 0.25; the means differ, so check the oracle against numpy instead
+    grid = np.linspace(-0.5, 0.5, 101)
+    rms_np = [np.sqrt(np.mean((np.interp(tf + d, ts, Fs) / Fs.mean() - Ff / Ff.mean()) ** 2)) for d in grid]
+    do, ro = orc.calibrate_delay(tf, Ff, ts, Fs, 0.5, 101)
+    assert do == pytest.approx(grid[int(np.argmin(rms_np))], abs=1e-12) and ro == pytest.approx(min(rms_np), rel=1e-10)
+    # a shift that leaves fewer than max(4, n/2) points is skipped; nothing qualifies -> rms = inf
+    assert orc.calibrate_delay(tf, Ff, ts + 100.0, Fs, 0.5, 11)[1] == math.inf
+    assert lc.calibrate_delay(tf, Ff, ts + 100.0, Fs, 0.5, 11) == (0.0, math.inf)
 
 
 def _free_port():
