@@ -6,6 +6,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <limits>
 #include <new>
 
 #include "../../include/raptor.h"
@@ -186,6 +187,17 @@ static void build_kp(raptor_ctx* c) {
         const double d1 = (p.x1_max - p.x1_min) / p.n1;
         k.x1_first = p.x1_min + 0.5 * d1; k.inv_d1 = 1.0 / d1;
     }
+    // pre-rejection range of the plasma sampler (KP::samp_r_lo/hi): a superset of where the exact tests can succeed
+    k.samp_r_lo = 0.0; k.samp_r_hi = std::numeric_limits<double>::infinity();
+    if ((p.plasma_model == M_GRID2D || p.plasma_model == M_GRID3DT) && p.n1 > 0) {
+        const double d1 = (p.x1_max - p.x1_min) / p.n1;
+        k.samp_r_lo = (p.mks_r0 + std::exp(k.x1_first)) * (1.0 - 1e-9);
+        k.samp_r_hi = (p.mks_r0 + std::exp(k.x1_first + (p.n1 - 1) * d1)) * (1.0 + 1e-9);
+    } else if (p.plasma_model == M_TORUS) {
+        k.samp_r_lo = std::max(0.0, (p.model[1] - std::fabs(p.model[2])) * (1.0 - 1e-9));
+        k.samp_r_hi = (p.model[1] + std::fabs(p.model[2])) * (1.0 + 1e-9);
+    }
+    k.r0_nz = p.mks_r0 != 0.0 ? 1 : 0;
     k.t0 = p.t0; k.inv_dt = p.dt_snap > 0.0 ? 1.0 / p.dt_snap : 0.0;
     k.grid = c->d_grid; k.freq = c->d_freq;
     k.nx = p.nx; k.ny = p.ny; k.integrator = p.integrator; k.step_policy = p.step_policy; k.max_steps = p.max_steps; k.n_freq = p.n_freq;

@@ -17,9 +17,6 @@
 
 namespace raptor {
 
-#ifndef RAPTOR_FASTPATH
-#define RAPTOR_FASTPATH 0
-#endif
 #ifndef RAPTOR_REFRESH
 #define RAPTOR_REFRESH 63      // library exp / sincos at the base point every (RAPTOR_REFRESH + 1)-th step
 #endif
@@ -65,7 +62,8 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
                 tmin = sTau[0];
                 for (int k = 1; k < P.n_freq; ++k) tmin = fmin(tmin, sTau[k * sstride]);
             }
-            if (tmin > P.tau_cutoff) { st = S_THICK; break; }
+            // tau >= 0: ordered like its bit pattern; a NaN compares false as in the floating-point test
+            if (pos_lt(P.tau_cutoff, tmin) && !pos_lt(__longlong_as_double(0x7ff0000000000000LL), tmin)) { st = S_THICK; break; }
         }
         const double h = step_size(P, G, X[2], K[1], K[2], K[3]);
         const double dl = -h;                                                  // backward [A2]
@@ -74,68 +72,10 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         const double hl = 0.5 * dl;
         Geom Gs;                        // geometry of the last stage point: the new base point is reached from it
         double t1, t2;                  // new point minus that stage point (x1, x2)
-        bool have_G = false;            // the step already produced the geometry of the new point
-#if RAPTOR_FASTPATH
-        if (INTEG == I_RK4) {
-            // Straight-line step for the common case (9 of 10 steps): the polynomial tiers are fixed in advance --
-            // stage 2 and stage 4 from the base point with the tier-1 polynomials, stage 3 and the new point with the
-            // tier-0 ones -- so the whole step is one basic block the compiler can schedule (the stage-4 geometry
-            // overlaps the stage-3 right-hand side), and the bounds are VERIFIED afterwards on the integer pipe; a step
-            // that breaks one is redone by the tiered code below from the untouched (X, K, G).
-            const double ca = H1 ? kPI : 2.0 * kPI;
-            const double d12 = hl * K[1], d22 = hl * K[2], an2 = ca * d22;
-            // stage 4 lies about twice as far from the base point as stage 2: enter with a factor 2 of room
-            if (abs_hi(d12) < kTier1DHi - 0x00100000 && abs_hi(an2) < kTier1AHi - 0x00100000) {
-                double f0, f1, f2, f3, k0, k1, k2, k3, a0, a1, a2, a3, s0 = 0.0, s1, s2, s3 = 0.0;
-                Geom G2, G3, G4, Gn;
-                geodesic_rhs(P, G, K[0], K[1], K[2], K[3], f0, f1, f2, f3);
-                a0 = f0; a1 = f1; a2 = f2; a3 = f3;
-                k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-                const double hh = hl * hl;
-                const double e1 = hh * f1, e2 = hh * f2, ane = ca * e2;
-                geom_shift_tier<H1, 5, 3, 3>(P, G, d12, d22, an2, G2);
-                geodesic_rhs(P, G2, k0, k1, k2, k3, f0, f1, f2, f3);
-                if (FULLX) { s0 = a0 + f0; s3 = a3 + f3; }
-                s1 = a1 + f1; s2 = a2 + f2;
-                a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
-                const double g1 = hl * f1, g2 = hl * f2;
-                k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-                const double d14 = dl * k1, d24 = dl * k2, an4 = ca * d24;
-                geom_shift_tier<H1, 3, 1, 2>(P, G2, e1, e2, ane, G3);
-                geom_shift_tier<H1, 5, 3, 3>(P, G, d14, d24, an4, G4);
-                geodesic_rhs(P, G3, k0, k1, k2, k3, f0, f1, f2, f3);
-                if (FULLX) { s0 += f0; s3 += f3; }
-                s1 += f1; s2 += f2;
-                a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
-                k0 = fma(dl, f0, K[0]); k1 = fma(dl, f1, K[1]); k2 = fma(dl, f2, K[2]); k3 = fma(dl, f3, K[3]);
-                geodesic_rhs(P, G4, k0, k1, k2, k3, f0, f1, f2, f3);
-                a0 += f0; a1 += f1; a2 += f2; a3 += f3;
-                const double d6 = dl * (1.0 / 6.0);
-                const double u1 = dl * fma(d6, s1, -g1), u2 = dl * fma(d6, s2, -g2), anu = ca * u2;
-                const bool refresh = ((n + 1) & RAPTOR_REFRESH) == 0;          // warp-uniform
-                if (!refresh) geom_shift_tier<H1, 3, 1, 2>(P, G4, u1, u2, anu, Gn);
-                const bool ok = (abs_hi(e1) < kTier0Hi) & (abs_hi(ane) < kTier0Hi) & (abs_hi(d14) < kTier1DHi) &
-                                (abs_hi(an4) < kTier1AHi) & (abs_hi(u1) < kTier0Hi) & (abs_hi(anu) < kTier0Hi);
-                if (ok) {
-                    if (FULLX) { X[0] = fma(dl, fma(d6, s0, K[0]), X[0]); X[3] = fma(dl, fma(d6, s3, K[3]), X[3]); }
-                    X[1] = fma(dl, fma(d6, s1, K[1]), X[1]); X[2] = fma(dl, fma(d6, s2, K[2]), X[2]);
-                    K[0] = fma(d6, a0, K[0]); K[1] = fma(d6, a1, K[1]); K[2] = fma(d6, a2, K[2]); K[3] = fma(d6, a3, K[3]);
-                    if (!refresh) G = Gn;
-                    have_G = true;
-                } else {
-                    // rare (a few steps per ray next to the hole): the base-point geometry is re-evaluated rather than
-                    // kept in registers across the whole straight-line step
-                    Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T;
-                }
-            }
-        }
-        if (INTEG == I_RK4 && have_G) {
-        } else
-#endif
         if (INTEG == I_RK4) {
             double f0, f1, f2, f3;          // stage acceleration
             double k0, k1, k2, k3;          // stage wavevector
-            double a0, a1, a2, a3;          // f_1 + 2 f_2 + 2 f_3 + f_4
+            double a0, a1, a2, a3;          // t, phi: f_1 + 2 f_2 + 2 f_3 + f_4; x1, x2: f_1 until the end
             double s0 = 0.0, s1, s2, s3 = 0.0;   // f_1 + f_2 + f_3   (components t, phi only with FULLX)
             Geom Gt;
             // stage 1 at (X, K)
@@ -143,38 +83,37 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             a0 = f0; a1 = f1; a2 = f2; a3 = f3;
             // stage 2 at X + dl/2 K, K + dl/2 f_1
             k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-            const double hh = hl * hl;
-            const double e1 = hh * f1, e2 = hh * f2;                               // stage-3 point minus stage-2 point
-            {
-                const double d1 = hl * K[1], d2 = hl * K[2];
-                geom_shift<H1>(P, G, X[1], X[2], d1, d2, Gs);
-            }
+            const double d12 = hl * K[1], d22 = hl * K[2];                         // stage-2 point minus X
+            geom_shift<H1>(P, G, X[1], X[2], d12, d22, Gs);
+            // stage-3 point minus stage-2 point: dl/2 (k_2 - K) = (dl/2)^2 f_1
+            const double e1 = fma(hl, k1, -d12), e2 = fma(hl, k2, -d22);
             const double x1s2 = fma(hl, K[1], X[1]), x2s2 = fma(hl, K[2], X[2]);   // stage-2 point (library fallback only)
             geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
             if (FULLX) { s0 = a0 + f0; s3 = a3 + f3; }
             s1 = a1 + f1; s2 = a2 + f2;
-            a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
-            const double g1 = hl * f1, g2 = hl * f2;                               // dl/2 f_2 (x1, x2): end-point offset below
+            a0 = fma(2.0, f0, a0); a3 = fma(2.0, f3, a3);
             // stage 3 at X + dl/2 k_2, K + dl/2 f_2
             k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
             geom_shift<H1>(P, Gs, x1s2, x2s2, e1, e2, Gt);
             geodesic_rhs(P, Gt, k0, k1, k2, k3, f0, f1, f2, f3);
             if (FULLX) { s0 += f0; s3 += f3; }
             s1 += f1; s2 += f2;
-            a0 = fma(2.0, f0, a0); a1 = fma(2.0, f1, a1); a2 = fma(2.0, f2, a2); a3 = fma(2.0, f3, a3);
+            a0 = fma(2.0, f0, a0); a3 = fma(2.0, f3, a3);
             // stage 4 at X + dl k_3, K + dl f_3
-            {
-                const double d1 = dl * k1, d2 = dl * k2;
-                geom_shift<H1>(P, G, X[1], X[2], d1, d2, Gs);
-            }
+            const double d14 = dl * k1, d24 = dl * k2;                             // stage-4 point minus X
+            geom_shift<H1>(P, G, X[1], X[2], d14, d24, Gs);
             k0 = fma(dl, f0, K[0]); k1 = fma(dl, f1, K[1]); k2 = fma(dl, f2, K[2]); k3 = fma(dl, f3, K[3]);
             geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
-            a0 += f0; a1 += f1; a2 += f2; a3 += f3;
+            // f_1 + 2 f_2 + 2 f_3 + f_4: t, phi accumulated; x1, x2 from the sum the position update needs anyway,
+            // 2 (f_1 + f_2 + f_3) + (f_4 - f_1)
+            a0 += f0; a3 += f3;
+            a1 = fma(2.0, s1, f1 - a1); a2 = fma(2.0, s2, f2 - a2);
             const double d6 = dl * (1.0 / 6.0);
-            // new point minus stage-4 point: dl (K + dl/6 S) - dl k_3 = dl (dl/6 S - dl/2 f_2)
-            t1 = dl * fma(d6, s1, -g1); t2 = dl * fma(d6, s2, -g2);
-            if (FULLX) { X[0] = fma(dl, fma(d6, s0, K[0]), X[0]); X[3] = fma(dl, fma(d6, s3, K[3]), X[3]); }     // Eq. 15
-            X[1] = fma(dl, fma(d6, s1, K[1]), X[1]); X[2] = fma(dl, fma(d6, s2, K[2]), X[2]);
+            const double w1 = fma(d6, s1, K[1]), w2 = fma(d6, s2, K[2]);           // Eq. 15: X' = X + dl (K + dl/6 S)
+            // new point minus stage-4 point: dl (K + dl/6 S) - dl k_3
+            t1 = fma(dl, w1, -d14); t2 = fma(dl, w2, -d24);
+            if (FULLX) { X[0] = fma(dl, fma(d6, s0, K[0]), X[0]); X[3] = fma(dl, fma(d6, s3, K[3]), X[3]); }
+            X[1] = fma(dl, w1, X[1]); X[2] = fma(dl, w2, X[2]);
             K[0] = fma(d6, a0, K[0]); K[1] = fma(d6, a1, K[1]); K[2] = fma(d6, a2, K[2]); K[3] = fma(d6, a3, K[3]);   // Eq. 16
         } else if (INTEG == I_RK2) {
             // "RK2" of Table B.1, read as the explicit midpoint method [A17]
@@ -220,7 +159,6 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         // incremental from stage 4; re-evaluated with the library functions every (RAPTOR_REFRESH+1)-th step so
         // that the round-off of the increments cannot accumulate (n is warp-uniform: a tile's lanes start together)
         if ((n & RAPTOR_REFRESH) == 0) { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
-        else if (have_G) { }
         else if (INTEG == I_VERLET || INTEG == I_VERLET_C) G = Gs;
         else geom_shift<H1, true>(P, Gs, X[1], X[2], t1, t2, G);
         if (MON) {
