@@ -94,7 +94,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             a0 = fma(2.0, f0, a0); a3 = fma(2.0, f3, a3);
             // stage 3 at X + dl/2 k_2, K + dl/2 f_2
             k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-            geom_shift<H1>(P, Gs, x1s2, x2s2, e1, e2, Gt);
+            geom_shift<H1, false, true>(P, Gs, x1s2, x2s2, e1, e2, Gt);
             geodesic_rhs(P, Gt, k0, k1, k2, k3, f0, f1, f2, f3);
             if (FULLX) { s0 += f0; s3 += f3; }
             s1 += f1; s2 += f2;
@@ -160,7 +160,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         // that the round-off of the increments cannot accumulate (n is warp-uniform: a tile's lanes start together)
         if ((n & RAPTOR_REFRESH) == 0) { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
         else if (INTEG == I_VERLET || INTEG == I_VERLET_C) G = Gs;
-        else geom_shift<H1, true>(P, Gs, X[1], X[2], t1, t2, G);
+        else geom_shift<H1, true, true>(P, Gs, X[1], X[2], t1, t2, G);
         if (MON) {
             Met M;
             met_eval(P, G, M);
