@@ -37,7 +37,8 @@ namespace raptor {
 // --------------------------------------------------------------------------------------------
 // MON: also evaluate the null condition g_mn k^m k^n (Eq. 4) at the new point of every step and keep
 // its largest magnitude along the ray (8(a) a3 "null-condition check"); diagnostics, built with FULLX only.
-template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG, bool MON>
+// R0: the chart has r0 != 0 (A.10); every contract configuration has r0 = 0, for which r = e^x1 costs nothing.
+template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG, bool MON, bool R0>
 __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta, double t_cam, double* __restrict__ sI,
                                           double* __restrict__ sTau, int sstride, double& I0, double& tau0,
                                           double X[4], double K[4], int& status, int& nsteps, int& nsampled, double& null_max) {
@@ -71,7 +72,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         if (MODEL == M_DISK) { x1p = X[1]; x2p = X[2]; Kp[0] = K[0]; Kp[1] = K[1]; Kp[2] = K[2]; Kp[3] = K[3]; }
         const double hl = 0.5 * dl;
         Geom Gs;                        // geometry of the last stage point: the new base point is reached from it
-        double t1, t2;                  // new point minus that stage point (x1, x2)
+        double t1, t2;                  // new point minus that stage point: x1 offset, x2 offset as an angle (shift_angle)
         if (INTEG == I_RK4) {
             double f0, f1, f2, f3;          // stage acceleration
             double k0, k1, k2, k3;          // stage wavevector
@@ -83,10 +84,12 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             a0 = f0; a1 = f1; a2 = f2; a3 = f3;
             // stage 2 at X + dl/2 K, K + dl/2 f_1
             k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-            const double d12 = hl * K[1], d22 = hl * K[2];                         // stage-2 point minus X
-            geom_shift<H1>(P, G, X[1], X[2], d12, d22, Gs);
+            // x2 offsets as angles (2 pi d2, or pi d2 for h = 1): ahl = c dl/2, al = c dl
+            const double al = shift_angle<H1>(dl), ahl = 0.5 * al;
+            const double d12 = hl * K[1], g22 = ahl * K[2];                        // stage-2 point minus X
+            geom_shift<H1, R0>(P, G, X[1], X[2], d12, g22, Gs);
             // stage-3 point minus stage-2 point: dl/2 (k_2 - K) = (dl/2)^2 f_1
-            const double e1 = fma(hl, k1, -d12), e2 = fma(hl, k2, -d22);
+            const double e1 = fma(hl, k1, -d12), e2 = fma(ahl, k2, -g22);
             const double x1s2 = fma(hl, K[1], X[1]), x2s2 = fma(hl, K[2], X[2]);   // stage-2 point (library fallback only)
             geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
             if (FULLX) { s0 = a0 + f0; s3 = a3 + f3; }
@@ -94,14 +97,14 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             a0 = fma(2.0, f0, a0); a3 = fma(2.0, f3, a3);
             // stage 3 at X + dl/2 k_2, K + dl/2 f_2
             k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
-            geom_shift<H1, false, true>(P, Gs, x1s2, x2s2, e1, e2, Gt);
+            geom_shift<H1, R0, false, true>(P, Gs, x1s2, x2s2, e1, e2, Gt);
             geodesic_rhs(P, Gt, k0, k1, k2, k3, f0, f1, f2, f3);
             if (FULLX) { s0 += f0; s3 += f3; }
             s1 += f1; s2 += f2;
             a0 = fma(2.0, f0, a0); a3 = fma(2.0, f3, a3);
             // stage 4 at X + dl k_3, K + dl f_3
-            const double d14 = dl * k1, d24 = dl * k2;                             // stage-4 point minus X
-            geom_shift<H1>(P, G, X[1], X[2], d14, d24, Gs);
+            const double d14 = dl * k1, g24 = al * k2;                             // stage-4 point minus X
+            geom_shift<H1, R0>(P, G, X[1], X[2], d14, g24, Gs);
             k0 = fma(dl, f0, K[0]); k1 = fma(dl, f1, K[1]); k2 = fma(dl, f2, K[2]); k3 = fma(dl, f3, K[3]);
             geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
             // f_1 + 2 f_2 + 2 f_3 + f_4: t, phi accumulated; x1, x2 from the sum the position update needs anyway,
@@ -111,7 +114,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             const double d6 = dl * (1.0 / 6.0);
             const double w1 = fma(d6, s1, K[1]), w2 = fma(d6, s2, K[2]);           // Eq. 15: X' = X + dl (K + dl/6 S)
             // new point minus stage-4 point: dl (K + dl/6 S) - dl k_3
-            t1 = fma(dl, w1, -d14); t2 = fma(dl, w2, -d24);
+            t1 = fma(dl, w1, -d14); t2 = fma(al, w2, -g24);
             if (FULLX) { X[0] = fma(dl, fma(d6, s0, K[0]), X[0]); X[3] = fma(dl, fma(d6, s3, K[3]), X[3]); }
             X[1] = fma(dl, w1, X[1]); X[2] = fma(dl, w2, X[2]);
             K[0] = fma(d6, a0, K[0]); K[1] = fma(d6, a1, K[1]); K[2] = fma(d6, a2, K[2]); K[3] = fma(d6, a3, K[3]);   // Eq. 16
@@ -121,10 +124,10 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             geodesic_rhs(P, G, K[0], K[1], K[2], K[3], f0, f1, f2, f3);
             k0 = fma(hl, f0, K[0]); k1 = fma(hl, f1, K[1]); k2 = fma(hl, f2, K[2]); k3 = fma(hl, f3, K[3]);
             const double d1 = hl * K[1], d2 = hl * K[2];
-            geom_shift<H1>(P, G, X[1], X[2], d1, d2, Gs);
+            geom_shift<H1, R0>(P, G, X[1], X[2], d1, shift_angle<H1>(d2), Gs);
             geodesic_rhs(P, Gs, k0, k1, k2, k3, f0, f1, f2, f3);
             // new point minus midpoint: dl k_mid - dl/2 K
-            t1 = fma(dl, k1, -d1); t2 = fma(dl, k2, -d2);
+            t1 = fma(dl, k1, -d1); t2 = shift_angle<H1>(fma(dl, k2, -d2));
             if (FULLX) { X[0] = fma(dl, k0, X[0]); X[3] = fma(dl, k3, X[3]); }
             X[1] = fma(dl, k1, X[1]); X[2] = fma(dl, k2, X[2]);
             K[0] = fma(dl, f0, K[0]); K[1] = fma(dl, f1, K[1]); K[2] = fma(dl, f2, K[2]); K[3] = fma(dl, f3, K[3]);
@@ -138,7 +141,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             if (FULLX) { X[0] += fma(hd2, f0, dl * K[0]); X[3] += fma(hd2, f3, dl * K[3]); }
             X[1] += t1; X[2] += t2;
             p0 = fma(dl, f0, K[0]); p1 = fma(dl, f1, K[1]); p2 = fma(dl, f2, K[2]); p3 = fma(dl, f3, K[3]);   // Eq. 18
-            geom_shift<H1, true>(P, G, X[1], X[2], t1, t2, Gs);
+            geom_shift<H1, R0, true>(P, G, X[1], X[2], t1, shift_angle<H1>(t2), Gs);
             geodesic_rhs(P, Gs, p0, p1, p2, p3, g0, g1, g2, g3);                                // Eq. 19
             p0 = fma(hl, f0 + g0, K[0]); p1 = fma(hl, f1 + g1, K[1]);                           // Eq. 20
             p2 = fma(hl, f2 + g2, K[2]); p3 = fma(hl, f3 + g3, K[3]);
@@ -160,7 +163,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
         // that the round-off of the increments cannot accumulate (n is warp-uniform: a tile's lanes start together)
         if ((n & RAPTOR_REFRESH) == 0) { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
         else if (INTEG == I_VERLET || INTEG == I_VERLET_C) G = Gs;
-        else geom_shift<H1, true, true>(P, Gs, X[1], X[2], t1, t2, G);
+        else geom_shift<H1, R0, true, true>(P, Gs, X[1], X[2], t1, t2, G);                 // t2: an angle
         if (MON) {
             Met M;
             met_eval(P, G, M);
@@ -213,7 +216,7 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
 // --------------------------------------------------------------------------------------------
 // Persistent-warp driver: tiles of 8x4 pixels (render) or 32 consecutive rays (trace) from a global queue.
 // --------------------------------------------------------------------------------------------
-template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG, bool MON>
+template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG, bool MON, bool R0>
 __global__ void __launch_bounds__(MULTI ? RAPTOR_BLOCK_MULTI : RAPTOR_BLOCK, MULTI ? (RAPTOR_BLOCK * RAPTOR_MIN_BLOCKS) / RAPTOR_BLOCK_MULTI : RAPTOR_MIN_BLOCKS)
 k_render(const __grid_constant__ KP P, const RenderOut O) {
     extern __shared__ double smem[];
@@ -260,7 +263,7 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
         if (active) {
             double X[4], K[4], I0, tau0, nmax;
             int status, n, ns;
-            trace_ray<MODEL, H1, MULTI, FULLX, INTEG, MON>(P, alpha, beta, t_cam, sI, sTau, sstride, I0, tau0, X, K, status, n, ns, nmax);
+            trace_ray<MODEL, H1, MULTI, FULLX, INTEG, MON, R0>(P, alpha, beta, t_cam, sI, sTau, sstride, I0, tau0, X, K, status, n, ns, nmax);
             steps += (unsigned)n; sampled += (unsigned)ns; rays += 1;
             const size_t npix = O.alpha ? (size_t)O.nrays : (size_t)P.nx * P.ny;
             if (O.image) {
@@ -296,10 +299,10 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
     }
 }
 
-template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG, bool MON = false>
+template <int MODEL, bool H1, bool MULTI, bool FULLX, int INTEG, bool MON, bool R0>
 static cudaError_t launch_one(const KP& P, const RenderOut& O, int grid, int block, cudaStream_t stream) {
     size_t smem = MULTI ? (size_t)2 * P.n_freq * block * sizeof(double) : 0;
-    auto kern = k_render<MODEL, H1, MULTI, FULLX, INTEG, MON>;
+    auto kern = k_render<MODEL, H1, MULTI, FULLX, INTEG, MON, R0>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -308,22 +311,22 @@ static cudaError_t launch_one(const KP& P, const RenderOut& O, int grid, int blo
     return cudaGetLastError();
 }
 
-template <int MODEL, bool FULLX, int INTEG>
+template <int MODEL, bool FULLX, int INTEG, bool MON, bool R0>
 static cudaError_t launch_hm(const KP& P, const RenderOut& O, bool h1, bool multi, int grid, int block, cudaStream_t s) {
-    if (FULLX && O.null_max) {           // per-step null monitor: the FULLX kernels with MON
-        if (h1) return multi ? launch_one<MODEL, true, true, FULLX, INTEG, FULLX>(P, O, grid, block, s) : launch_one<MODEL, true, false, FULLX, INTEG, FULLX>(P, O, grid, block, s);
-        return multi ? launch_one<MODEL, false, true, FULLX, INTEG, FULLX>(P, O, grid, block, s) : launch_one<MODEL, false, false, FULLX, INTEG, FULLX>(P, O, grid, block, s);
-    }
-    if (h1) return multi ? launch_one<MODEL, true, true, FULLX, INTEG>(P, O, grid, block, s) : launch_one<MODEL, true, false, FULLX, INTEG>(P, O, grid, block, s);
-    return multi ? launch_one<MODEL, false, true, FULLX, INTEG>(P, O, grid, block, s) : launch_one<MODEL, false, false, FULLX, INTEG>(P, O, grid, block, s);
+    if (h1) return multi ? launch_one<MODEL, true, true, FULLX, INTEG, MON, R0>(P, O, grid, block, s) : launch_one<MODEL, true, false, FULLX, INTEG, MON, R0>(P, O, grid, block, s);
+    return multi ? launch_one<MODEL, false, true, FULLX, INTEG, MON, R0>(P, O, grid, block, s) : launch_one<MODEL, false, false, FULLX, INTEG, MON, R0>(P, O, grid, block, s);
 }
 
 template <int MODEL, int INTEG>
 cudaError_t launch_model(const KP& P, const RenderOut& O, bool h1, bool multi, bool fullx, int grid, int block, cudaStream_t s) {
-    // the 3-D / slow-light sampler reads X^t, X^phi: always FULLX; the other models need them for the XK output only.
-    // The second-order integrators (8(f) f1) are built in the FULLX form only.
-    if (MODEL == M_GRID3DT || fullx || O.null_max || INTEG != I_RK4) return launch_hm<MODEL, true, INTEG>(P, O, h1, multi, grid, block, s);
-    return launch_hm<MODEL, MODEL == M_GRID3DT || INTEG != I_RK4, INTEG>(P, O, h1, multi, grid, block, s);
+    // The lean kernels (no X^t / X^phi, r0 = 0) serve RK4 on the models that do not read t, phi; everything else is
+    // FULLX: the 3-D / slow-light sampler reads X^t, X^phi, the trace output wants them, and the second-order
+    // integrators (8(f) f1) are built in that form only.  A chart with r0 != 0 and the per-step null monitor run on the
+    // general kernels (FULLX, R0; MON only there).
+    if (O.null_max) return launch_hm<MODEL, true, INTEG, true, true>(P, O, h1, multi, grid, block, s);
+    if (P.r0_nz) return launch_hm<MODEL, true, INTEG, false, true>(P, O, h1, multi, grid, block, s);
+    if (MODEL == M_GRID3DT || fullx || INTEG != I_RK4) return launch_hm<MODEL, true, INTEG, false, false>(P, O, h1, multi, grid, block, s);
+    return launch_hm<MODEL, MODEL == M_GRID3DT || INTEG != I_RK4, INTEG, false, false>(P, O, h1, multi, grid, block, s);
 }
 
 // one translation unit per (plasma model, integrator): -DRAPTOR_MODEL=m -DRAPTOR_INTEG=i (build.py, in parallel);

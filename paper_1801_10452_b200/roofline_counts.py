@@ -165,9 +165,9 @@ def load(path: str = DEFAULT_JSON):
 
 
 # mangled-name substrings of the kernels bench.py's workloads launch (for operand_forms)
-KERNEL_OF = {"C0": "k_renderILi1ELb1ELb0ELb0ELi0ELb0E", "C1": "k_renderILi2ELb1ELb0ELb0ELi0ELb0E",
-             "C2": "k_renderILi3ELb0ELb0ELb0ELi0ELb0E", "C3": "k_renderILi3ELb0ELb1ELb0ELi0ELb0E",
-             "C4": "k_renderILi4ELb0ELb0ELb1ELi0ELb0E", "PB1": "k_renderILi3ELb0ELb0ELb1ELi3ELb0E"}
+KERNEL_OF = {"C0": "k_renderILi1ELb1ELb0ELb0ELi0ELb0ELb0E", "C1": "k_renderILi2ELb1ELb0ELb0ELi0ELb0ELb0E",
+             "C2": "k_renderILi3ELb0ELb0ELb0ELi0ELb0ELb0E", "C3": "k_renderILi3ELb0ELb1ELb0ELi0ELb0ELb0E",
+             "C4": "k_renderILi4ELb0ELb0ELb1ELi0ELb0ELb0E", "PB1": "k_renderILi3ELb0ELb0ELb1ELi3ELb0ELb0E"}
 
 
 def main(argv):
