@@ -50,22 +50,17 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
     }
     int n = 0, ns = 0, ncross = 0, st = S_RUNNING;
     double nmax = 0.0;
+    // tau cut-off: the optical depths change on sampled steps only, so the comparison with the cut-off is made there
+    // and the loop head tests a flag (same exit, same step count: the head tests run in the oracle's order)
+    bool thick = P.use_tau_cutoff && 0.0 > P.tau_cutoff;
     Geom G;
     { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
+    bool fin = true;                    // the state after the last step is finite
     for (;;) {
-        // [A7]; r = r0 + e^x1 is positive (or +inf): compared on the integer pipe
-        if (pos_lt(G.r, P.r_in)) { st = S_CAPTURED; break; }
-        if (pos_lt(P.r_out, G.r)) { st = S_ESCAPED; break; }
-        if (n >= P.max_steps) { st = S_MAXSTEPS; break; }
-        if (P.use_tau_cutoff) {
-            double tmin = tau;
-            if (MULTI) {
-                tmin = sTau[0];
-                for (int k = 1; k < P.n_freq; ++k) tmin = fmin(tmin, sTau[k * sstride]);
-            }
-            // tau >= 0: ordered like its bit pattern; a NaN compares false as in the floating-point test
-            if (pos_lt(P.tau_cutoff, tmin) && !pos_lt(__longlong_as_double(0x7ff0000000000000LL), tmin)) { st = S_THICK; break; }
-        }
+        // the exits of the loop as ONE branch (which of them it was is sorted out after the loop, in the order of [A7]:
+        // non-finite state right after the step, then horizon, escape, step cap, optical-depth cap at the head of the
+        // next iteration); r = r0 + e^x1 is positive (or +inf): compared on the integer pipe
+        if (!fin | pos_lt(G.r, P.r_in) | pos_lt(P.r_out, G.r) | (n >= P.max_steps) | thick) break;
         const double h = step_size(P, G, X[2], K[1], K[2], K[3]);
         const double dl = -h;                                                  // backward [A2]
         double x1p = 0.0, x2p = 0.0, Kp[4] = {0.0, 0.0, 0.0, 0.0};             // thin disk: state before the step
@@ -154,17 +149,21 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             t1 = 0.0; t2 = 0.0;                                                                 // Gs is the new point
         }
         ++n;
-        bool fin = is_finite_bits(X[1]) & is_finite_bits(X[2]) &
-                   is_finite_bits(K[0]) & is_finite_bits(K[1]) & is_finite_bits(K[2]) & is_finite_bits(K[3]);
-        if (FULLX) fin = fin & is_finite_bits(X[0]) & is_finite_bits(X[3]);
-        if (!fin) { st = S_NONFINITE; break; }
+        // RK4: a non-finite X' = X + dl (K + dl/6 S) means a non-finite S (K was finite on entry), and then K' = K + dl/6 (2 S + f_4 - f_1)
+        // (or its t, phi form) is non-finite too: testing K' alone is the same test
+        fin = is_finite_bits(K[0]) & is_finite_bits(K[1]) & is_finite_bits(K[2]) & is_finite_bits(K[3]);
+        if (INTEG != I_RK4) {
+            fin = fin & is_finite_bits(X[1]) & is_finite_bits(X[2]);
+            if (FULLX) fin = fin & is_finite_bits(X[0]) & is_finite_bits(X[3]);
+        }
+        // a non-finite state leaves the loop at its head; until then it must not be sampled or monitored
         // ---- new point: geometry shared by transfer, termination, step rule and the next stage 1 ----
         // incremental from stage 4; re-evaluated with the library functions every (RAPTOR_REFRESH+1)-th step so
         // that the round-off of the increments cannot accumulate (n is warp-uniform: a tile's lanes start together)
         if ((n & RAPTOR_REFRESH) == 0) { Geom T; geom_eval_call<H1>(P.r0, P.omh, X[1], X[2], &T); G = T; }
         else if (INTEG == I_VERLET || INTEG == I_VERLET_C) G = Gs;
         else geom_shift<H1, R0, true, true>(P, Gs, X[1], X[2], t1, t2, G);                 // t2: an angle
-        if (MON) {
+        if (MON && fin) {
             Met M;
             met_eval(P, G, M);
             const double kr = G.ex * K[1], kh = G.dth * K[2];
@@ -174,12 +173,12 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
             // I = sum of g^p / r^2 over the counted crossings, tau = g of the first counted one
             double dI, gg;
             bool counted;
-            if (disk_crossing(P, x1p, x2p, Kp, X, K, ncross + 1, dI, gg, counted)) {
+            if (fin && disk_crossing(P, x1p, x2p, Kp, X, K, ncross + 1, dI, gg, counted)) {
                 ++ncross;
-                if (counted) { I += dI; if (ns == 0) tau = gg; ++ns; }
+                if (counted) { I += dI; if (ns == 0) tau = gg; ++ns; if (P.use_tau_cutoff) thick = tau > P.tau_cutoff; }
             }
         } else
-        if (MODEL != M_VACUUM && !pos_lt(G.r, P.r_in) && !pos_lt(P.r_out, G.r)) {   // [A8] end-point sample
+        if (MODEL != M_VACUUM && fin && !pos_lt(G.r, P.r_in) && !pos_lt(P.r_out, G.r)) {   // [A8] end-point sample
             Plasma pl;
             if (plasma_sample<MODEL>(P, G, X, K[0], G.ex * K[1], G.dth * K[2], K[3], pl)) {
                 ++ns;
@@ -206,9 +205,19 @@ __device__ __forceinline__ void trace_ray(const KP& P, double alpha, double beta
                 } else {
                     transfer_one(pl, E, __ldg(P.freq), __ldg(P.freq + 1), __ldg(P.freq + 2), I, tau);
                 }
+                if (P.use_tau_cutoff) {
+                    double tmin = tau;
+                    if (MULTI) {
+                        tmin = sTau[0];
+                        for (int k = 1; k < P.n_freq; ++k) tmin = fmin(tmin, sTau[k * sstride]);
+                    }
+                    thick = tmin > P.tau_cutoff;                               // false for a NaN
+                }
             }
         }
     }
+    st = !fin ? S_NONFINITE : pos_lt(G.r, P.r_in) ? S_CAPTURED : pos_lt(P.r_out, G.r) ? S_ESCAPED
+       : n >= P.max_steps ? S_MAXSTEPS : S_THICK;
     I0 = I; tau0 = tau; null_max = nmax;
     status = st; nsteps = n; nsampled = ns;
 }

@@ -70,7 +70,8 @@ def test_create_destroy_does_not_leak_device_memory(rb):
             img = torch.empty((1, 16, 16), dtype=torch.float64, device="cuda")
             flux = torch.empty((1,), dtype=torch.float64, device="cuda")
             rb.raptor_spectrum(ctx, flux.data_ptr(), None, None)        # allocates the scratch image
-            rb.raptor_render_host(ctx, np.empty((1, 16, 16)).ctypes.data, None, None, None)
+            host = np.empty((1, 16, 16))                                # kept alive until the call has returned
+            rb.raptor_render_host(ctx, host.ctypes.data, None, None, None)
             rb.raptor_destroy(ctx)
 
     cycle(3)                                                     # warm up allocator pools (cudaMallocAsync, torch)
