@@ -561,8 +561,11 @@ def test_per_step_null_monitor_matches_the_oracle(rb, orc, cfg):
         plain = R.trace(al, be)
         g = R.trace(al, be, monitor_null=True)
         end_norm = np.abs(R.null_norm(g["XK"]))
-    # the monitoring kernel is the same integration: identical results
-    assert np.array_equal(plain["nsteps"], g["nsteps"]) and np.array_equal(plain["I"], g["I"]) and np.array_equal(plain["XK"], g["XK"])
+    # the monitoring kernel is the same integration: identical step counts and end states; the intensities agree to
+    # rounding (two instantiations of the same arithmetic: where the compiler contracts a product and a sum of the
+    # sampler into one FMA may differ between them once the monitor's metric evaluation sits next to the sampler's)
+    assert np.array_equal(plain["nsteps"], g["nsteps"]) and np.array_equal(plain["XK"], g["XK"])
+    assert np.allclose(plain["I"], g["I"], rtol=1e-12, atol=0.0)
     o = orc.Oracle(s)
     ring = 0
     peaked = 0
