@@ -151,6 +151,72 @@ def operand_forms(source_csv: str, lib_path: str, mangled: str, steps_per_launch
     return out_counts
 
 
+def by_function(disasm: str, source_csv: str, mangled: str, steps_per_launch: float) -> dict:
+    """FP64-pipe and all warp instructions per warp-step by device function: where a step's instructions go.
+
+    ``disasm`` = ``nvdisasm -g -c`` of a cubin of the kernel built with the library's flags, e.g.
+
+        nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -std=c++17 --fmad=true -DRAPTOR_MODEL=3 -DRAPTOR_INTEG=0 \
+             -cubin paper_1801_10452_b200/csrc/raptor_render.cu -o m3.cubin && nvdisasm -g -c m3.cubin > m3.dis
+
+    (its ``//## File ..., line N`` marks name the innermost inlined source line of every instruction);
+    ``source_csv`` = ``ncu -i prof.ncu-rep --page source --csv --print-source sass`` of one launch of that kernel (executed
+    count per SASS instruction).  The two listings are joined by instruction order (the opcodes must agree), lines of
+    raptor_device.cuh are mapped to the ``__device__`` function they lie in, everything in raptor_render.cu is the RK4
+    combination and the loop.  Run:  python -m paper_1801_10452_b200.roofline_counts --by-function m3.dis source_C2.csv
+    k_renderILi3ELb0ELb0ELb0ELi0ELb0ELb0E <accepted steps of the launch>."""
+    import re
+    starts = []
+    with open(os.path.join(CSRC, "raptor_device.cuh")) as fh:
+        for i, line in enumerate(fh, 1):
+            m = re.match(r"^(?:static )?__device__ .*?(\w+)\(", line)
+            if m:
+                starts.append((i, m.group(1)))
+
+    def func_of(path, line):
+        if path.endswith("raptor_device.cuh"):
+            name = "?"
+            for s0, n0 in starts:
+                if s0 <= line:
+                    name = n0
+            return name
+        return "raptor_render.cu" if path.endswith("raptor_render.cu") else "library:" + os.path.basename(path)
+
+    ins, take, path, line = [], False, "?", 0
+    with open(disasm) as fh:
+        for text in fh:
+            if text.startswith("//---") and ".text." in text:
+                take = mangled in text
+                continue
+            if not take:
+                continue
+            m = re.match(r'\s*//## File "(.*)", line (\d+)', text)
+            if m:
+                path, line = m.group(1), int(m.group(2))
+                continue
+            m = re.match(r"\s*/\*([0-9a-f]{4,})\*/\s+(.*?);", text)
+            if m:
+                op = re.sub(r"^@!?U?P\d+\s+", "", m.group(2).strip()).split()[0].split(".")[0]
+                ins.append((op, func_of(path, line)))
+    with open(source_csv, newline="") as fh:
+        rows = list(csv.reader(fh))
+    head = next(r for r in rows if "Source" in r and "Instructions Executed" in r)
+    i_s, i_e = head.index("Source"), head.index("Instructions Executed")
+    prof = [(r[i_s].strip(), int(r[i_e])) for r in rows[rows.index(head) + 1:] if len(r) > i_e and r[i_e].isdigit()]
+    n = min(len(ins), len(prof))
+    mismatch = sum(1 for (op, _), (src, _) in zip(ins[:n], prof[:n])
+                   if op != re.sub(r"^@!?U?P\d+\s+", "", src).split()[0].split(".")[0])
+    warp_steps = steps_per_launch / 32.0
+    out = {}
+    for (op, fn), (_, cnt) in zip(ins[:n], prof[:n]):
+        row = out.setdefault(fn, {"all": 0.0, "fp64_pipe": 0.0})
+        row["all"] += cnt / warp_steps
+        if op in ("DFMA", "DMUL", "DADD", "DSETP", "DMNMX"):
+            row["fp64_pipe"] += cnt / warp_steps
+    out["_listing"] = {"instructions": n, "mismatch": mismatch}
+    return out
+
+
 def load(path: str = DEFAULT_JSON):
     """(table, None) if the committed counts belong to the sources in this tree, else (None, reason)."""
     if not os.path.exists(path):
@@ -171,6 +237,11 @@ KERNEL_OF = {"C0": "k_renderILi1ELb1ELb0ELb0ELi0ELb0ELb0E", "C1": "k_renderILi2E
 
 
 def main(argv):
+    if len(argv) > 1 and argv[1] == "--by-function":
+        table = by_function(argv[2], argv[3], argv[4], float(argv[5]))
+        for fn, row in sorted(table.items(), key=lambda kv: -kv[1].get("all", 0.0)):
+            print(f"{fn:28s} " + "  ".join(f"{k} {v:9.1f}" if isinstance(v, float) else f"{k} {v}" for k, v in row.items()))
+        return
     run_dir = argv[1] if len(argv) > 1 else "gpurun_out"
     out = argv[2] if len(argv) > 2 else DEFAULT_JSON
     table = collect(run_dir)
