@@ -8,6 +8,8 @@
 #include <cstring>
 #include <limits>
 #include <new>
+#include <utility>
+#include <vector>
 
 #include "../../include/raptor.h"
 #include "raptor_kernels.h"
@@ -29,6 +31,7 @@ struct raptor_ctx {
     double* d_freq = nullptr;
     double nu0 = 0.0;                      // first frequency (precision = 1 has exactly one)
     unsigned int* d_queue = nullptr;
+    unsigned int* d_order = nullptr;       // tiles of one image sorted by the distance of their centre from the image centre
     unsigned long long* d_counters = nullptr;
     double* d_partial = nullptr;      // flux partial sums [n_freq][chunks]
     double* d_profile_partial = nullptr;   // line-profile partial sums [nbins][chunks]
@@ -255,6 +258,21 @@ extern "C" int raptor_create(const raptor_params* p, raptor_ctx** out) {
         CKC(cudaMemcpy(c->d_freq, tab, sizeof(double) * 3 * p->n_freq, cudaMemcpyHostToDevice));
     }
     CKC(cudaMalloc(&c->d_queue, sizeof(unsigned int)));
+    {
+        // launch order of the 8x4-pixel tiles: by the impact parameter of the tile centre, nearest first (ties: by index)
+        const int ntx = (p->nx + 7) / 8, nty = (p->ny + 3) / 4;
+        std::vector<std::pair<double, unsigned>> key((size_t)ntx * nty);
+        for (int ty = 0; ty < nty; ++ty)
+            for (int tx = 0; tx < ntx; ++tx) {
+                const double al = ((tx * 8 + 4.0) / p->nx - 0.5) * p->fov_M, be = ((ty * 4 + 2.0) / p->ny - 0.5) * p->fov_M;
+                key[(size_t)ty * ntx + tx] = {al * al + be * be, (unsigned)(ty * ntx + tx)};
+            }
+        std::sort(key.begin(), key.end());
+        std::vector<unsigned> order(key.size());
+        for (size_t i = 0; i < key.size(); ++i) order[i] = key[i].second;
+        CKC(cudaMalloc(&c->d_order, sizeof(unsigned) * order.size()));
+        CKC(cudaMemcpy(c->d_order, order.data(), sizeof(unsigned) * order.size(), cudaMemcpyHostToDevice));
+    }
     CKC(cudaMalloc(&c->d_counters, 3 * sizeof(unsigned long long)));
     CKC(cudaMemset(c->d_counters, 0, 3 * sizeof(unsigned long long)));
     const size_t npix = (size_t)p->nx * p->ny;
@@ -300,6 +318,7 @@ static int mark(raptor_ctx* ctx, cudaStream_t s) {
 
 static int run_rays(raptor_ctx* ctx, RenderOut& O, cudaStream_t s) {
     O.queue = ctx->d_queue;
+    O.order = O.alpha ? nullptr : ctx->d_order;
     O.counters = ctx->d_counters;
     if (O.frames <= 1) O.null_max = ctx->d_null_max;
     if (O.tile_stride == 0) { O.tile_offset = 0; O.tile_stride = 1; }
@@ -662,7 +681,7 @@ extern "C" int raptor_fp64_probe(int32_t form, int32_t iters, double* warp_inst_
 
 extern "C" int raptor_destroy(raptor_ctx* ctx) {
     if (!ctx) return RAPTOR_OK;
-    cudaFree(ctx->d_grid); cudaFree(ctx->d_grid_f32); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_counters);
+    cudaFree(ctx->d_grid); cudaFree(ctx->d_grid_f32); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_order); cudaFree(ctx->d_counters);
     cudaFree(ctx->d_partial); cudaFree(ctx->d_profile_partial); cudaFree(ctx->d_lc_partial); cudaFree(ctx->d_scratch_image); cudaFree(ctx->d_scratch_flux);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);

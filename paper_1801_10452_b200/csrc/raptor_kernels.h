@@ -24,6 +24,7 @@ struct RenderOut {
     unsigned int* queue;            // tile counter, zeroed before the launch
     unsigned int ntiles;            // tiles this launch processes: global tile = tile_offset + i * tile_stride
     unsigned int tile_offset, tile_stride;
+    const unsigned int* order;      // [tiles of one image] tile (ty * ntx + tx) of sequence number k: from the image centre outward; NULL: by rows
     unsigned long long* counters;   // [3] steps, sampled steps, rays (accumulated)
     const double* alpha;            // trace mode: explicit impact parameters [nrays]; NULL = render the pixel grid
     const double* beta;
