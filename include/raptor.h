@@ -165,12 +165,12 @@ int raptor_calibrate_delay(int32_t n_fast, const double *t_fast, const double *F
                            const double *F_slow, double max_shift, int32_t n_grid, double *delay, double *rms);
 
 /* Multi-GPU sharding of one image: after this call raptor_render / raptor_spectrum /
- * raptor_render_host trace only the 8x4-pixel tiles at positions rank, rank + world, rank + 2 world, ... of the
- * kernel's tile sequence (rows of tiles from the image centre outward -- mid, mid - 1, mid + 1, ... with
- * mid = ceil(ny/4) / 2 -- and left to right within a row) and leave every other pixel of the caller's output buffers untouched.  Rays are independent, so the ranks'
+ * raptor_render_host trace only the 8x4-pixel tiles whose raster index ty * ceil(nx/8) + tx is rank modulo world
+ * (interleaved, so that shadow and torus are spread evenly; the kernel launches them nearest to the image centre first)
+ * and leave every other pixel of the caller's output buffers untouched.  Rays are independent, so the ranks'
  * images (zero-initialised by the caller) sum to the full image exactly.  Where the library owns the image
  * (raptor_spectrum with a NULL image, raptor_render_host) it zeroes it first, so fluxes are the shard's own and
- * sum to the full flux.  Default (0, 1) = whole image. */
+ * sum to the full flux.  Default (0, 1) = whole image.  Synchronises the device (the shard's tile table is replaced). */
 int raptor_set_shard(raptor_ctx *ctx, int32_t rank, int32_t world);
 
 /* Render + flux reduction: d_flux_jy device [n_freq], F_k = 1e23 sum_pix I_k (fov/nx)(fov/ny) L^2/D^2 [Jy],

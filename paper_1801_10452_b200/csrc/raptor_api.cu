@@ -32,6 +32,8 @@ struct raptor_ctx {
     double nu0 = 0.0;                      // first frequency (precision = 1 has exactly one)
     unsigned int* d_queue = nullptr;
     unsigned int* d_order = nullptr;       // tiles of one image sorted by the distance of their centre from the image centre
+    unsigned int* d_order_shard = nullptr; // the same for this rank's tiles (tile index mod world == rank), raptor_set_shard
+    std::vector<unsigned> order_host;
     unsigned long long* d_counters = nullptr;
     double* d_partial = nullptr;      // flux partial sums [n_freq][chunks]
     double* d_profile_partial = nullptr;   // line-profile partial sums [nbins][chunks]
@@ -271,7 +273,9 @@ extern "C" int raptor_create(const raptor_params* p, raptor_ctx** out) {
         std::vector<unsigned> order(key.size());
         for (size_t i = 0; i < key.size(); ++i) order[i] = key[i].second;
         CKC(cudaMalloc(&c->d_order, sizeof(unsigned) * order.size()));
+        CKC(cudaMalloc(&c->d_order_shard, sizeof(unsigned) * order.size()));
         CKC(cudaMemcpy(c->d_order, order.data(), sizeof(unsigned) * order.size(), cudaMemcpyHostToDevice));
+        c->order_host.swap(order);
     }
     CKC(cudaMalloc(&c->d_counters, 3 * sizeof(unsigned long long)));
     CKC(cudaMemset(c->d_counters, 0, 3 * sizeof(unsigned long long)));
@@ -319,6 +323,10 @@ static int mark(raptor_ctx* ctx, cudaStream_t s) {
 static int run_rays(raptor_ctx* ctx, RenderOut& O, cudaStream_t s) {
     O.queue = ctx->d_queue;
     O.order = O.alpha ? nullptr : ctx->d_order;
+    if (O.order && ctx->shard_world > 1 && O.tile_stride == (unsigned)ctx->shard_world) {
+        // a shard owns the tiles whose index is rank mod world; it launches them in the same nearest-first order
+        O.order = ctx->d_order_shard; O.tile_offset = 0; O.tile_stride = 1;
+    }
     O.counters = ctx->d_counters;
     if (O.frames <= 1) O.null_max = ctx->d_null_max;
     if (O.tile_stride == 0) { O.tile_offset = 0; O.tile_stride = 1; }
@@ -502,6 +510,13 @@ extern "C" int raptor_set_shard(raptor_ctx* ctx, int32_t rank, int32_t world) {
     if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
     if (world < 1 || rank < 0 || rank >= world) return fail(ctx, RAPTOR_EINVAL, "shard: need 0 <= rank < world");
     ctx->shard_rank = rank; ctx->shard_world = world;
+    if (world > 1) {
+        std::vector<unsigned> mine;
+        for (unsigned t : ctx->order_host)
+            if (t % (unsigned)world == (unsigned)rank) mine.push_back(t);
+        CK(ctx, cudaDeviceSynchronize());            // a launch in flight may still read the previous table
+        if (!mine.empty()) CK(ctx, cudaMemcpy(ctx->d_order_shard, mine.data(), sizeof(unsigned) * mine.size(), cudaMemcpyHostToDevice));
+    }
     return RAPTOR_OK;
 }
 
@@ -681,7 +696,7 @@ extern "C" int raptor_fp64_probe(int32_t form, int32_t iters, double* warp_inst_
 
 extern "C" int raptor_destroy(raptor_ctx* ctx) {
     if (!ctx) return RAPTOR_OK;
-    cudaFree(ctx->d_grid); cudaFree(ctx->d_grid_f32); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_order); cudaFree(ctx->d_counters);
+    cudaFree(ctx->d_grid); cudaFree(ctx->d_grid_f32); cudaFree(ctx->d_freq); cudaFree(ctx->d_queue); cudaFree(ctx->d_order); cudaFree(ctx->d_order_shard); cudaFree(ctx->d_counters);
     cudaFree(ctx->d_partial); cudaFree(ctx->d_profile_partial); cudaFree(ctx->d_lc_partial); cudaFree(ctx->d_scratch_image); cudaFree(ctx->d_scratch_flux);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);

@@ -19,27 +19,17 @@ def n_tiles(nx: int, ny: int) -> int:
     return ((nx + TILE_X - 1) // TILE_X) * ((ny + TILE_Y - 1) // TILE_Y)
 
 
-def tile_row_of_position(k: int, nty: int) -> int:
-    """The kernel's tile order walks the rows of tiles from the image centre outward: position 0, 1, 2, ... of the
-    sequence is row mid, mid - 1, mid + 1, ... (mid = nty // 2), so that the longest rays start first."""
-    mid = nty // 2
-    return mid - 1 - k // 2 if k % 2 else mid + k // 2
-
-
 def tiles_of_rank(nx: int, ny: int, rank: int, world: int) -> range:
-    """Positions in the kernel's tile sequence (rows centre-outward, left to right within a row) traced by ``rank``
-    after raptor_set_shard(rank, world)."""
+    """Tiles (raster index ty * ntx + tx) traced by ``rank`` after raptor_set_shard(rank, world): those whose index is
+    rank mod world.  The kernel launches them nearest to the image centre first; the order does not change the image."""
     return range(rank, n_tiles(nx, ny), world)
 
 
 def pixel_owner_map(nx: int, ny: int, world: int) -> torch.Tensor:
     """[ny, nx] int32: which rank traces each pixel under the tile sharding."""
-    ntx, nty = (nx + TILE_X - 1) // TILE_X, (ny + TILE_Y - 1) // TILE_Y
-    mid = nty // 2
+    ntx = (nx + TILE_X - 1) // TILE_X
     iy, ix = torch.meshgrid(torch.arange(ny), torch.arange(nx), indexing="ij")
-    ty = iy // TILE_Y
-    pos = torch.where(ty >= mid, 2 * (ty - mid), 2 * (mid - 1 - ty) + 1)        # inverse of tile_row_of_position
-    return ((pos * ntx + ix // TILE_X) % world).to(torch.int32)
+    return (((iy // TILE_Y) * ntx + ix // TILE_X) % world).to(torch.int32)
 
 
 def frames_of_rank(n_frames: int, rank: int, world: int) -> range:

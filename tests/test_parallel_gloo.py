@@ -67,19 +67,15 @@ def test_two_rank_sharding_and_aggregation():
     assert sorted(results[0][4] + results[1][4]) == list(range(7))
 
 
-def test_tile_rows_run_from_the_centre_outward():
-    for nty in (1, 2, 5, 8, 256):
-        rows = [parallel.tile_row_of_position(k, nty) for k in range(nty)]
-        assert sorted(rows) == list(range(nty))
-        assert rows[0] == nty // 2 and all(abs(a - nty // 2) <= abs(b - nty // 2) + 1 for a, b in zip(rows, rows[1:]))
-    # the owner map is the inverse of that walk: position p = k * ntx + tx belongs to rank p % world
+def test_owner_map_is_the_raster_tile_index_mod_world():
+    # raptor_set_shard(rank, world): tile (tx, ty) of the 8x4-pixel tiling belongs to rank (ty * ntx + tx) % world
     nx, ny, world = 52, 38, 3
     owner = parallel.pixel_owner_map(nx, ny, world)
     ntx, nty = 7, 10
-    for k in range(nty):
-        ty = parallel.tile_row_of_position(k, nty)
+    for ty in range(nty):
         for tx in range(ntx):
-            assert int(owner[min(4 * ty, ny - 1), 8 * tx]) == (k * ntx + tx) % world
+            assert int(owner[min(4 * ty, ny - 1), 8 * tx]) == (ty * ntx + tx) % world
+            assert int(owner[min(4 * ty + 3, ny - 1), min(8 * tx + 7, nx - 1)]) == (ty * ntx + tx) % world
 
 
 def test_tiles_are_dealt_exactly_once():
