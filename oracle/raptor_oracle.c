@@ -29,6 +29,8 @@
  * cyclotron frequency the paper prints, multilinear-interpolation exactness,
  * both step rules (Eq. 21-24 and the configs[0] clamp with and without the polar guard), the
  * optical-depth cut-off exit, pixel centres and the [k][iy][ix] image layout by hand computation.
+ * The fluid-frame block (nu_hat, pitch angle, field seeds, sampling guard) is pinned THROUGH orc_transfer /
+ * orc_trace_ray against aberration, Doppler and gravitational-redshift closed forms (tests/test_oracle_fluid_frame.py).
  * Parity unpinned (definitions, not derivable -- see DESIGN.md): the VALUES of the step-rule
  * constants of BASELINE.json configs[0] and of eps_polar, the end-point sampling of the quadrature
  * [A8], the amplitudes of the synthetic plasma models, and Table 3 / Fig. 7-13 of the paper
