@@ -180,6 +180,35 @@ int raptor_spectrum(raptor_ctx *ctx, double *d_flux_jy, double *d_image_or_null,
 /* Flux reduction alone of an image already on the device. */
 int raptor_flux(raptor_ctx *ctx, const double *d_image, double *d_flux_jy, void *cuda_stream);
 
+/* Flux reduction for callers that must not allocate device memory (same sum as raptor_flux: Fig. 2 units,
+ * PAPER.md:248; F_k = scale * sum_pix I_k, fixed order).
+ *
+ * Who needs it: raptor_flux wants a context, and raptor_create takes its buffers from cudaMalloc.  That is not open to
+ * everybody -- a plug-in whose host program has already given the whole device to its own memory pool, a job with a
+ * device-memory budget fixed in advance, a loop that cannot afford cudaMalloc's device-wide synchronisation, or code
+ * that merely holds an image on the device and has no context at all.  This call needs no context and calls neither
+ * cudaMalloc nor cudaFree nor any library routine that allocates: the partial sums of the reduction sit in an array
+ * that is part of the library image (128 KiB on every GPU that loads the library, held until the process exits).
+ *
+ *   d_image   device, [n_planes][npix] float64 (for an image of raptor_render: n_planes = n_freq, npix = ny * nx)
+ *   scale     factor applied to each sum; raptor_flux uses 1e23 (fov/nx)(fov/ny) L^2/D^2 for Jy, 1 gives plain sums
+ *   d_flux    device, [n_planes] float64, written on the stream
+ * Limit: n_planes * ceil(npix / 16384) <= RAPTOR_FLUX_STATIC_MAX_PARTIALS (e.g. 64 planes of 2048 x 2048 pixels);
+ * anything larger, npix = 0, n_planes < 1 or a NULL buffer returns RAPTOR_EINVAL with the numbers in the message
+ * (raptor_last_error(NULL)), and nothing is launched.  For the same image and scale the result equals raptor_flux's
+ * bit for bit.
+ *
+ * The first call on each device looks up the device address of the array (one cudaGetSymbolAddress, which may also
+ * make the driver load the library's code onto that device); make that first call once per device during start-up,
+ * with the device current, before any stream capture begins.  Later calls only launch two kernels on the stream.
+ * All calls on one device share the one array: it keeps what the last call left, which is harmless because every
+ * element a call reads it has written itself first -- but two calls that can run on the GPU at the same time
+ * (different streams, no ordering between them) race on it and both results are then undefined.  Keep the calls of a
+ * device on one stream or order them with events. */
+#define RAPTOR_FLUX_STATIC_MAX_PARTIALS 16384
+int raptor_flux_static(const double *d_image, uint64_t npix, int32_t n_planes, double scale, double *d_flux,
+                       void *cuda_stream);
+
 /* End-to-end convenience with HOST buffers: render on the context's own stream (after every earlier call on
  * this context has finished, see "Ordering"), copy image ([n_freq][ny][nx]), optional status / nsteps ([ny][nx])
  * and optional flux ([n_freq]) back, synchronise.  Under a shard the pixels of other ranks' tiles come back 0. */

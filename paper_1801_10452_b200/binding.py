@@ -23,7 +23,7 @@ STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 
 # every symbol include/raptor.h declares
 SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_render_disk",
            "raptor_line_profile", "raptor_set_camera_time", "raptor_set_window", "raptor_upload_snapshot",
-           "raptor_light_curve", "raptor_calibrate_delay", "raptor_spectrum", "raptor_flux",
+           "raptor_light_curve", "raptor_calibrate_delay", "raptor_spectrum", "raptor_flux", "raptor_flux_static",
            "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_null_norm", "raptor_set_null_monitor", "raptor_get_counters", "raptor_fp64_peak", "raptor_fp64_probe",
            "raptor_destroy", "raptor_last_error")
 
@@ -80,6 +80,7 @@ def lib():
         L.raptor_line_profile.argtypes = [vp, vp, vp, i32, C.c_double, C.c_double, vp, vp]
         L.raptor_spectrum.argtypes = [vp, vp, vp, vp]
         L.raptor_flux.argtypes = [vp, vp, vp, vp]
+        L.raptor_flux_static.argtypes = [vp, C.c_uint64, i32, C.c_double, vp, vp]
         L.raptor_render_host.argtypes = [vp, vp, vp, vp, vp]
         L.raptor_trace.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
         L.raptor_eval_rhs.argtypes = [vp, i32, vp, vp, vp]
@@ -190,6 +191,12 @@ def raptor_spectrum(ctx, d_flux, d_image=None, stream=None):
 
 def raptor_flux(ctx, d_image, d_flux, stream=None):
     _check(lib().raptor_flux(ctx, d_image, d_flux, stream), ctx)
+
+
+def raptor_flux_static(d_image, npix, n_planes, scale, d_flux, stream=None):
+    """Flux reduction without a context and without any device allocation (raptor.h): for callers that may not
+    call cudaMalloc.  d_image [n_planes][npix] and d_flux [n_planes] are device addresses owned by the caller."""
+    _check(lib().raptor_flux_static(d_image, int(npix), int(n_planes), float(scale), d_flux, stream))
 
 
 def raptor_render_host(ctx, h_image, h_status=None, h_nsteps=None, h_flux=None):

@@ -18,7 +18,7 @@ LIB = os.path.join(HERE, "libraptor_b200.so")
 N_MODELS = 7
 N_INTEG = 4
 HEADERS = ["raptor_device.cuh", "raptor_kernels.h", os.path.join("..", "..", "include", "raptor.h")]
-SOURCES = ["raptor_render.cu", "raptor_render_f32.cu", "raptor_kernels.cu", "raptor_api.cu"]
+SOURCES = ["raptor_render.cu", "raptor_render_f32.cu", "raptor_kernels.cu", "raptor_flux_static.cu", "raptor_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC"]
 
@@ -48,7 +48,7 @@ def build(force: bool = False, verbose: bool = False, extra: list[str] | None = 
             o = os.path.join(objdir, f"raptor_render_m{m}_i{i}.o")
             jobs.append((base + [f"-DRAPTOR_MODEL={m}", f"-DRAPTOR_INTEG={i}", "-c",
                                  os.path.join(CSRC, "raptor_render.cu"), "-o", o], o))
-    for src in ("raptor_kernels.cu", "raptor_api.cu", "raptor_render_f32.cu"):
+    for src in ("raptor_kernels.cu", "raptor_flux_static.cu", "raptor_api.cu", "raptor_render_f32.cu"):
         o = os.path.join(objdir, src.replace(".cu", ".o"))
         jobs.append((base + ["-c", os.path.join(CSRC, src), "-o", o], o))
     with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 1)) as pool:

@@ -536,6 +536,23 @@ extern "C" int raptor_flux(raptor_ctx* ctx, const double* d_image, double* d_flu
     return mark(ctx, (cudaStream_t)cuda_stream);
 }
 
+// The reduction of raptor_flux for callers that cannot allocate (include/raptor.h): no context, partial sums in the
+// library's own __device__ array (raptor_flux_static.cu).  Nothing here or below it calls cudaMalloc / cudaFree.
+static_assert(RAPTOR_FLUX_STATIC_MAX_PARTIALS == kFluxStaticSlots, "header limit and array size must agree");
+extern "C" int raptor_flux_static(const double* d_image, uint64_t npix, int32_t n_planes, double scale, double* d_flux,
+                                  void* cuda_stream) {
+    if (!d_image || !d_flux) return fail(nullptr, RAPTOR_EINVAL, "raptor_flux_static: NULL buffer");
+    if (npix == 0 || n_planes < 1) return fail(nullptr, RAPTOR_EINVAL, "raptor_flux_static: need npix >= 1 and n_planes >= 1");
+    const uint64_t chunks = (npix + 16383) / 16384;
+    if (chunks > (uint64_t)kFluxStaticSlots || chunks * (uint64_t)n_planes > (uint64_t)kFluxStaticSlots)
+        return fail(nullptr, RAPTOR_EINVAL,
+                    "raptor_flux_static: %d planes x %llu chunks of 16384 pixels = %llu partial sums, the built-in scratch holds %d "
+                    "(use raptor_flux, which allocates, for larger images)",
+                    n_planes, (unsigned long long)chunks, (unsigned long long)(chunks * (uint64_t)n_planes), kFluxStaticSlots);
+    CK(nullptr, launch_flux_static(d_image, (size_t)npix, n_planes, scale, d_flux, (cudaStream_t)cuda_stream));
+    return RAPTOR_OK;
+}
+
 static int ensure_scratch(raptor_ctx* ctx) {
     const size_t need = (size_t)ctx->p.nx * ctx->p.ny * ctx->p.n_freq;
     if (ctx->scratch_pixels < need) {

@@ -64,6 +64,10 @@ cudaError_t launch_profile(const double* d_image, const double* d_red, size_t np
                            double scale, double* d_partial, double* d_hist, cudaStream_t stream);
 cudaError_t launch_null_norm(const KP& P, int n, const double* d_XK, double* d_out, double* d_elq, cudaStream_t stream);
 cudaError_t launch_eval_rhs(const KP& P, int n, const double* d_XK, double* d_f, cudaStream_t stream);
+// raptor_flux_static.cu: the same reduction with its partial sums in a __device__ array of the library (no allocation)
+constexpr int kFluxStaticSlots = 16384;      // partial sums the array holds: n_planes * flux_chunks(npix) must fit
+cudaError_t launch_flux_static(const double* d_image, size_t npix, int n_planes, double scale, double* d_flux,
+                               cudaStream_t stream);
 cudaError_t launch_fp64_peak(int iters, int blocks, double* d_out, cudaStream_t stream);
 cudaError_t launch_fp64_form(int mode, int iters, int blocks, double* d_out, cudaStream_t stream);
 
