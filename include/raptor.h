@@ -26,7 +26,7 @@
 extern "C" {
 #endif
 
-#define RAPTOR_ABI_VERSION 2u
+#define RAPTOR_ABI_VERSION 3u
 
 enum {
     RAPTOR_OK = 0,
@@ -160,7 +160,8 @@ int raptor_light_curve(raptor_ctx *ctx, int32_t n_frames, double t_cam0, double 
  * slow-light curve is interpolated linearly at t_fast[i] + d_k (points outside [t_slow[0], t_slow[n_slow-1]] are
  * left out; a shift that keeps fewer than max(4, n_fast/2) points is skipped) and the rms difference to the
  * fast-light curve is formed; *delay receives the first shift with the smallest rms, *rms that rms (+inf and
- * delay 0 if every shift was skipped).  HOST pointers, t_slow ascending; plain host arithmetic, synchronous. */
+ * delay 0 if every shift was skipped).  HOST pointers; plain host arithmetic, synchronous.  RAPTOR_EINVAL if t_slow is
+ * not strictly ascending or the mean of either curve is zero or not finite. */
 int raptor_calibrate_delay(int32_t n_fast, const double *t_fast, const double *F_fast, int32_t n_slow, const double *t_slow,
                            const double *F_slow, double max_shift, int32_t n_grid, double *delay, double *rms);
 
@@ -173,11 +174,13 @@ int raptor_calibrate_delay(int32_t n_fast, const double *t_fast, const double *F
  * sum to the full flux.  Default (0, 1) = whole image.  Synchronises the device (the shard's tile table is replaced). */
 int raptor_set_shard(raptor_ctx *ctx, int32_t rank, int32_t world);
 
-/* Render + flux reduction: d_flux_jy device [n_freq], F_k = 1e23 sum_pix I_k (fov/nx)(fov/ny) L^2/D^2 [Jy],
- * summed in a fixed order (deterministic).  d_image_or_null: as d_image, or NULL to use scratch. */
+/* Render + flux reduction (the spectra of Fig. 2, units PAPER.md:248, and the fluxes of Table 3):
+ * d_flux_jy device [n_freq], F_k = 1e23 sum_pix I_k (fov/nx)(fov/ny) L^2/D^2 [Jy] -- the pixel's solid angle as seen
+ * from distance D times its intensity -- summed in a fixed order (deterministic).  d_image_or_null: as d_image, or NULL
+ * to use scratch. */
 int raptor_spectrum(raptor_ctx *ctx, double *d_flux_jy, double *d_image_or_null, void *cuda_stream);
 
-/* Flux reduction alone of an image already on the device. */
+/* Flux reduction alone (same sum and units: Fig. 2; Table 3) of an image already on the device. */
 int raptor_flux(raptor_ctx *ctx, const double *d_image, double *d_flux_jy, void *cuda_stream);
 
 /* Flux reduction for callers that must not allocate device memory (same sum as raptor_flux: Fig. 2 units,
@@ -233,11 +236,16 @@ int raptor_null_norm(raptor_ctx *ctx, int32_t n, const double *d_XK, double *d_o
  * raptor_render_disk and raptor_trace also evaluate g_mn k^m k^n at the new point of EVERY step and write its largest
  * magnitude along each ray to d_null_max ([ny][nx], resp. [n]; device, caller-owned, must stay valid until unset).
  * A ray whose norm peaked near the horizon and recovered is visible here, not in the end state.  The default kernels
- * are unchanged; the monitoring variants cost about 5 % more.  NULL switches it off.  (raptor_light_curve ignores it.) */
-int raptor_set_null_monitor(raptor_ctx *ctx, double *d_null_max_or_null);
+ * are unchanged; the monitoring variants cost about 5 % more.  NULL switches it off.  (raptor_light_curve ignores it.)
+ * capacity = number of float64 elements the buffer holds (ignored for NULL): while the monitor is set, a call that would
+ * write more than that (an image of ny * nx > capacity pixels, a trace of n > capacity rays) returns RAPTOR_EINVAL and
+ * launches nothing -- a buffer sized for a trace and left set across a render cannot be overrun.  raptor_spectrum and
+ * raptor_render_host go through raptor_render and therefore monitor as well while it is set. */
+int raptor_set_null_monitor(raptor_ctx *ctx, double *d_null_max_or_null, uint64_t capacity);
 
-/* Counters accumulated by every render / trace since creation (synchronises the context's work):
- * accepted RK4 steps, steps on which plasma was sampled, rays traced. */
+/* Counters accumulated by every render / trace since creation: accepted integrator steps, steps on which plasma was
+ * sampled, rays traced.  Waits for the last call made on this context (not for the device: other streams keep
+ * running).  No passage of the paper: measurement (SURVEY.md 8(d) needs the step count of an image). */
 int raptor_get_counters(raptor_ctx *ctx, uint64_t *total_steps, uint64_t *sampled_steps, uint64_t *rays);
 
 /* Measures the FP64 FMA peak of the current device with independent DFMA chains on all SMs:
@@ -252,6 +260,7 @@ int raptor_fp64_peak(int32_t iters, double *tflops, double *ms);
  * (DESIGN.md 5.1): the bound of a kernel depends on its operand forms, not only on its instruction count. */
 int raptor_fp64_probe(int32_t form, int32_t iters, double *warp_inst_per_sec, double *sm_clock_hz);
 
+/* Releases the context and its device memory (NULL is allowed).  No passage of the paper: lifecycle. */
 int raptor_destroy(raptor_ctx *ctx);
 
 /* Message of the last failure on this context; ctx == NULL: of the last failed raptor_create /

@@ -14,7 +14,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libraptor_b200.so")
-ABI_VERSION = 2
+ABI_VERSION = 3
 MAX_FREQ = 64
 
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
@@ -85,7 +85,7 @@ def lib():
         L.raptor_trace.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
         L.raptor_eval_rhs.argtypes = [vp, i32, vp, vp, vp]
         L.raptor_null_norm.argtypes = [vp, i32, vp, vp, vp, vp]
-        L.raptor_set_null_monitor.argtypes = [vp, vp]
+        L.raptor_set_null_monitor.argtypes = [vp, vp, C.c_uint64]
         L.raptor_get_counters.argtypes = [vp, u64p, u64p, u64p]
         L.raptor_fp64_peak.argtypes = [i32, dp, dp]
         L.raptor_fp64_probe.argtypes = [i32, i32, dp, dp]
@@ -219,8 +219,9 @@ def raptor_null_norm(ctx, n, d_XK, d_out, d_ELQ=None, stream=None):
     _check(lib().raptor_null_norm(ctx, n, d_XK, d_out, d_ELQ, stream), ctx)
 
 
-def raptor_set_null_monitor(ctx, d_null_max=None):
-    _check(lib().raptor_set_null_monitor(ctx, d_null_max), ctx)
+def raptor_set_null_monitor(ctx, d_null_max=None, capacity=0):
+    """capacity: float64 elements the buffer holds; calls that would write more are refused while it is set (raptor.h)."""
+    _check(lib().raptor_set_null_monitor(ctx, d_null_max, int(capacity)), ctx)
 
 
 def raptor_get_counters(ctx):
@@ -361,7 +362,7 @@ class Raptor:
         nsteps = torch.empty((n,), dtype=torch.int32, device="cuda")
         nmax = torch.zeros((n,), dtype=torch.float64, device="cuda") if monitor_null else None
         if monitor_null:
-            raptor_set_null_monitor(self.ctx, nmax.data_ptr())
+            raptor_set_null_monitor(self.ctx, nmax.data_ptr(), n)
         try:
             raptor_trace(self.ctx, n, al.data_ptr(), be.data_ptr(), I.data_ptr(), tau.data_ptr(), XK.data_ptr(),
                          status.data_ptr(), nsteps.data_ptr(), _stream_ptr())

@@ -47,6 +47,7 @@ struct raptor_ctx {
     KPf kpf;                               // precision = 1
     float* d_grid_f32 = nullptr;           // precision = 1: (float) of d_grid
     double* d_null_max = nullptr;          // raptor_set_null_monitor: caller-owned output of the next render / trace calls
+    uint64_t null_max_capacity = 0;        // elements the caller said it holds
     cudaEvent_t ev_last = nullptr;         // recorded after every asynchronous call: raptor_render_host orders itself after it
     char err[512] = {0};
 };
@@ -329,6 +330,13 @@ static int run_rays(raptor_ctx* ctx, RenderOut& O, cudaStream_t s) {
     }
     O.counters = ctx->d_counters;
     if (O.frames <= 1) O.null_max = ctx->d_null_max;
+    if (O.null_max) {
+        // the monitor buffer was sized by the caller for one kind of call: refuse the call that would write past its end
+        const uint64_t need = O.alpha ? (uint64_t)O.nrays : (uint64_t)ctx->p.nx * (uint64_t)ctx->p.ny;
+        if (need > ctx->null_max_capacity)
+            return fail(ctx, RAPTOR_EINVAL, "null monitor buffer holds %llu elements, this call writes %llu: unset it or set a larger one",
+                        (unsigned long long)ctx->null_max_capacity, (unsigned long long)need);
+    }
     if (O.tile_stride == 0) { O.tile_offset = 0; O.tile_stride = 1; }
     CK(ctx, cudaMemsetAsync(ctx->d_queue, 0, sizeof(unsigned int), s));
     if (ctx->p.precision == 1) {
@@ -482,6 +490,10 @@ extern "C" int raptor_calibrate_delay(int32_t n_fast, const double* t_fast, cons
     for (int i = 0; i < n_fast; ++i) mf += F_fast[i];
     for (int i = 0; i < n_slow; ++i) ms += F_slow[i];
     mf /= n_fast; ms /= n_slow;
+    if (!(mf != 0.0) || !(ms != 0.0) || !std::isfinite(mf) || !std::isfinite(ms))
+        return fail(nullptr, RAPTOR_EINVAL, "raptor_calibrate_delay: the mean of a light curve is zero or not finite (curves are normalised by their means)");
+    for (int i = 1; i < n_slow; ++i)
+        if (!(t_slow[i] > t_slow[i - 1])) return fail(nullptr, RAPTOR_EINVAL, "raptor_calibrate_delay: t_slow must be strictly ascending (t_slow[%d] <= t_slow[%d])", i, i - 1);
     const int need = std::max(4, n_fast / 2);
     double best_d = 0.0, best = INFINITY;
     for (int k = 0; k < n_grid; ++k) {
@@ -509,7 +521,6 @@ extern "C" int raptor_calibrate_delay(int32_t n_fast, const double* t_fast, cons
 extern "C" int raptor_set_shard(raptor_ctx* ctx, int32_t rank, int32_t world) {
     if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
     if (world < 1 || rank < 0 || rank >= world) return fail(ctx, RAPTOR_EINVAL, "shard: need 0 <= rank < world");
-    ctx->shard_rank = rank; ctx->shard_world = world;
     if (world > 1) {
         std::vector<unsigned> mine;
         for (unsigned t : ctx->order_host)
@@ -517,12 +528,16 @@ extern "C" int raptor_set_shard(raptor_ctx* ctx, int32_t rank, int32_t world) {
         CK(ctx, cudaDeviceSynchronize());            // a launch in flight may still read the previous table
         if (!mine.empty()) CK(ctx, cudaMemcpy(ctx->d_order_shard, mine.data(), sizeof(unsigned) * mine.size(), cudaMemcpyHostToDevice));
     }
+    // only now: a failed upload above leaves the previous (rank, world) together with its own table
+    ctx->shard_rank = rank; ctx->shard_world = world;
     return RAPTOR_OK;
 }
 
-extern "C" int raptor_set_null_monitor(raptor_ctx* ctx, double* d_null_max_or_null) {
+extern "C" int raptor_set_null_monitor(raptor_ctx* ctx, double* d_null_max_or_null, uint64_t capacity) {
     if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
+    if (d_null_max_or_null && capacity == 0) return fail(ctx, RAPTOR_EINVAL, "null monitor: capacity must be >= 1 element");
     ctx->d_null_max = d_null_max_or_null;
+    ctx->null_max_capacity = d_null_max_or_null ? capacity : 0;
     return RAPTOR_OK;
 }
 
@@ -590,25 +605,32 @@ extern "C" int raptor_render_host(raptor_ctx* ctx, double* h_image, int32_t* h_s
     cudaStream_t s = ctx->own_stream;
     CK(ctx, cudaStreamWaitEvent(s, ctx->ev_last, 0));          // after every earlier call on this context (uploads, renders)
     int32_t *d_status = nullptr, *d_nsteps = nullptr;
-    if (h_status) CK(ctx, cudaMallocAsync(&d_status, npix * sizeof(int32_t), s));
-    if (h_nsteps) CK(ctx, cudaMallocAsync(&d_nsteps, npix * sizeof(int32_t), s));
+    // every CUDA call of the body goes through `step`, so that the two temporaries are released on every way out
+    cudaError_t ce = cudaSuccess;
+    const char* what = "";
+#define STEP(call) do { if (!rc && ce == cudaSuccess) { ce = (call); if (ce != cudaSuccess) what = #call; } } while (0)
+    if (h_status) STEP(cudaMallocAsync(&d_status, npix * sizeof(int32_t), s));
+    if (h_nsteps) STEP(cudaMallocAsync(&d_nsteps, npix * sizeof(int32_t), s));
     if (ctx->shard_world > 1) {                                // pixels of other ranks' tiles read as zero
-        CK(ctx, cudaMemsetAsync(ctx->d_scratch_image, 0, npix * ctx->p.n_freq * sizeof(double), s));
-        if (d_status) CK(ctx, cudaMemsetAsync(d_status, 0, npix * sizeof(int32_t), s));
-        if (d_nsteps) CK(ctx, cudaMemsetAsync(d_nsteps, 0, npix * sizeof(int32_t), s));
+        STEP(cudaMemsetAsync(ctx->d_scratch_image, 0, npix * ctx->p.n_freq * sizeof(double), s));
+        if (d_status) STEP(cudaMemsetAsync(d_status, 0, npix * sizeof(int32_t), s));
+        if (d_nsteps) STEP(cudaMemsetAsync(d_nsteps, 0, npix * sizeof(int32_t), s));
     }
-    rc = raptor_render(ctx, ctx->d_scratch_image, d_status, d_nsteps, s);
-    if (!rc && h_flux_jy) rc = raptor_flux(ctx, ctx->d_scratch_image, ctx->d_scratch_flux, s);
-    if (!rc) {
-        CK(ctx, cudaMemcpyAsync(h_image, ctx->d_scratch_image, npix * ctx->p.n_freq * sizeof(double), cudaMemcpyDeviceToHost, s));
-        if (h_status) CK(ctx, cudaMemcpyAsync(h_status, d_status, npix * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-        if (h_nsteps) CK(ctx, cudaMemcpyAsync(h_nsteps, d_nsteps, npix * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-        if (h_flux_jy) CK(ctx, cudaMemcpyAsync(h_flux_jy, ctx->d_scratch_flux, ctx->p.n_freq * sizeof(double), cudaMemcpyDeviceToHost, s));
-    }
+    if (ce == cudaSuccess) rc = raptor_render(ctx, ctx->d_scratch_image, d_status, d_nsteps, s);
+    if (ce == cudaSuccess && !rc && h_flux_jy) rc = raptor_flux(ctx, ctx->d_scratch_image, ctx->d_scratch_flux, s);
+    STEP(cudaMemcpyAsync(h_image, ctx->d_scratch_image, npix * ctx->p.n_freq * sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (h_status) STEP(cudaMemcpyAsync(h_status, d_status, npix * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    if (h_nsteps) STEP(cudaMemcpyAsync(h_nsteps, d_nsteps, npix * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+    if (h_flux_jy) STEP(cudaMemcpyAsync(h_flux_jy, ctx->d_scratch_flux, ctx->p.n_freq * sizeof(double), cudaMemcpyDeviceToHost, s));
+#undef STEP
     if (d_status) cudaFreeAsync(d_status, s);
     if (d_nsteps) cudaFreeAsync(d_nsteps, s);
-    CK(ctx, cudaStreamSynchronize(s));
-    return rc;
+    const cudaError_t se = cudaStreamSynchronize(s);
+    if (ce != cudaSuccess)
+        return fail(ctx, ce == cudaErrorMemoryAllocation ? RAPTOR_ENOMEM : RAPTOR_ECUDA, "%s: %s", what, cudaGetErrorString(ce));
+    if (rc) return rc;
+    CK(ctx, se);
+    return RAPTOR_OK;
 }
 
 extern "C" int raptor_trace(raptor_ctx* ctx, int32_t n, const double* d_alpha, const double* d_beta, double* d_I, double* d_tau,
@@ -643,8 +665,9 @@ extern "C" int raptor_null_norm(raptor_ctx* ctx, int32_t n, const double* d_XK, 
 extern "C" int raptor_get_counters(raptor_ctx* ctx, uint64_t* total_steps, uint64_t* sampled_steps, uint64_t* rays) {
     if (!ctx) return fail(nullptr, RAPTOR_EINVAL, "ctx is NULL");
     unsigned long long h[3];
-    CK(ctx, cudaDeviceSynchronize());
-    CK(ctx, cudaMemcpy(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost));
+    CK(ctx, cudaEventSynchronize(ctx->ev_last));     // the last call made on this context; other streams of the process keep running
+    CK(ctx, cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, ctx->own_stream));
+    CK(ctx, cudaStreamSynchronize(ctx->own_stream));
     if (total_steps) *total_steps = h[0];
     if (sampled_steps) *sampled_steps = h[1];
     if (rays) *rays = h[2];

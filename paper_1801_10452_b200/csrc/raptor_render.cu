@@ -258,18 +258,11 @@ k_render(const __grid_constant__ KP P, const RenderOut O) {
             alpha = active ? O.alpha[pix] : 0.0;
             beta = active ? O.beta[pix] : 0.0;
         } else {
-            // tile order: from the image centre outward: the longest rays (photon ring; under the step rule of Eq. 21-24
-            // everything near the hole) start first and the launch ends on the uniform outer tiles instead of waiting
-            // for a late long tile (rows from the centre row outward against row-major: PB1 -9 %, PB1 FP32 -15 %)
-            int tx, ty;
-            if (O.order) {                       // tiles sorted by the distance of their centre from the image centre
-                const unsigned t = __ldg(O.order + tile);
-                ty = (int)(t / (unsigned)ntx); tx = (int)(t - (unsigned)ty * (unsigned)ntx);
-            } else {                             // rows of tiles from the centre row outward
-                const int seq_row = tile / ntx, mid = ((P.ny + 3) >> 2) >> 1;
-                tx = tile - seq_row * ntx;
-                ty = (seq_row & 1) ? mid - 1 - (seq_row >> 1) : mid + (seq_row >> 1);
-            }
+            // tile order (O.order, built at raptor_create / raptor_set_shard): by the impact parameter of the tile centre,
+            // nearest first: the longest rays (photon ring; under the step rule of Eq. 21-24 everything near the hole)
+            // start first and the launch ends on the uniform outer tiles instead of waiting for a late long tile
+            const unsigned t = __ldg(O.order + tile);
+            const int ty = (int)(t / (unsigned)ntx), tx = (int)(t - (unsigned)ty * (unsigned)ntx);
             const int ix = (tx << 3) + (lane & 7), iy = (ty << 2) + (lane >> 3);
             active = ix < P.nx && iy < P.ny;
             alpha = fma((double)ix + 0.5, P.pix_dx, -0.5 * P.fov);             // pixel centres [A4b]

@@ -142,7 +142,7 @@ __device__ __forceinline__ float ks_dot(const Metf& M, float At, float Ar, float
 __device__ __forceinline__ bool transfer(const KPf& P, const Geomf& G, const float X[4], const float K[4], float h, float& I, float& tau) {
     float q[8];
     if (!grid2d_interp(P, X[1], X[2], q)) return false;
-    if (!(q[0] > 0.0f)) return false;
+    if (!(q[0] > 1e-30f && q[0] < 1e30f)) return false;      // positive normal density only: MUFU.RCP flushes denormals, maps huge to 0
     Metf M;
     M.ss = G.s * G.s; M.ass = P.a * M.ss; M.Sig = fmaf(G.r, G.r, P.a2 * G.c * G.c); M.rr = fmaf(G.r, G.r, P.a2);
     M.f = 2.0f * P.m * G.r * rcpf(M.Sig);
@@ -213,18 +213,11 @@ __global__ void __launch_bounds__(128) k_render_f32(const __grid_constant__ KPf 
             alpha = active ? (float)O.alpha[pix] : 0.0f;
             beta = active ? (float)O.beta[pix] : 0.0f;
         } else {
-            // tile order: from the image centre outward: the longest rays (photon ring; under the step rule of Eq. 21-24
-            // everything near the hole) start first and the launch ends on the uniform outer tiles instead of waiting
-            // for a late long tile (rows from the centre row outward against row-major: PB1 -9 %, PB1 FP32 -15 %)
-            int tx, ty;
-            if (O.order) {                       // tiles sorted by the distance of their centre from the image centre
-                const unsigned t = __ldg(O.order + tile);
-                ty = (int)(t / (unsigned)ntx); tx = (int)(t - (unsigned)ty * (unsigned)ntx);
-            } else {                             // rows of tiles from the centre row outward
-                const int seq_row = tile / ntx, mid = ((P.ny + 3) >> 2) >> 1;
-                tx = tile - seq_row * ntx;
-                ty = (seq_row & 1) ? mid - 1 - (seq_row >> 1) : mid + (seq_row >> 1);
-            }
+            // tile order (O.order, built at raptor_create / raptor_set_shard): by the impact parameter of the tile centre,
+            // nearest first: the longest rays (photon ring; under the step rule of Eq. 21-24 everything near the hole)
+            // start first and the launch ends on the uniform outer tiles instead of waiting for a late long tile
+            const unsigned t = __ldg(O.order + tile);
+            const int ty = (int)(t / (unsigned)ntx), tx = (int)(t - (unsigned)ty * (unsigned)ntx);
             const int ix = (tx << 3) + (lane & 7), iy = (ty << 2) + (lane >> 3);
             active = ix < P.nx && iy < P.ny;
             alpha = ((float)ix + 0.5f) * P.fov / (float)P.nx - 0.5f * P.fov;       // pixel centres [A4b]

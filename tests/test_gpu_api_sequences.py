@@ -148,3 +148,79 @@ def test_wien_tail_corner_of_the_planck_function(rb, orc, x):
             assert (r["tau"][0] > 1.0) == (x < 709.785)          # thick below the overflow, no absorption above
         assert g["I"][0, i] == pytest.approx(r["I"][0], rel=1e-10)
         assert g["tau"][0, i] == pytest.approx(r["tau"][0], rel=1e-10, abs=0.0)
+
+
+def test_null_monitor_buffer_cannot_be_overrun_by_a_larger_call(rb):
+    # the monitor pointer stays set across calls; a buffer sized for a 50-ray trace must not receive a 24 x 24 image
+    s = scenes.config_C1(24)
+    with rb.Raptor(s) as R:
+        small = torch.full((50 + 8,), -1.0, dtype=torch.float64, device="cuda")
+        rb.raptor_set_null_monitor(R.ctx, small.data_ptr(), 50)
+        al = torch.linspace(-9.0, 9.0, 50, dtype=torch.float64, device="cuda")
+        be = torch.full((50,), 0.7, dtype=torch.float64, device="cuda")
+        rb.raptor_trace(R.ctx, 50, al.data_ptr(), be.data_ptr())              # fits
+        with pytest.raises(rb.RaptorError) as err:
+            R.render()                                                         # 576 pixels into 50 elements: refused
+        assert err.value.code == rb.EINVAL and "null monitor" in str(err.value)
+        with pytest.raises(rb.RaptorError):
+            rb.raptor_trace(R.ctx, 51, al.data_ptr(), be.data_ptr())
+        with pytest.raises(rb.RaptorError):
+            R.spectrum()                                                       # goes through raptor_render
+        with pytest.raises(rb.RaptorError):
+            rb.raptor_set_null_monitor(R.ctx, small.data_ptr(), 0)
+        torch.cuda.synchronize()
+        got = small.cpu().numpy()
+        assert np.all(got[:50] >= 0.0) and np.all(got[50:] == -1.0)           # the trace wrote its 50, nothing went past
+        rb.raptor_set_null_monitor(R.ctx, None)
+        img0 = R.render(want_status=False)
+        big = torch.zeros((s.ny * s.nx,), dtype=torch.float64, device="cuda")
+        rb.raptor_set_null_monitor(R.ctx, big.data_ptr(), big.numel())
+        img1 = R.render(want_status=False)
+        rb.raptor_set_null_monitor(R.ctx, None)
+        torch.cuda.synchronize()
+        assert float(big.max()) > 0.0 and np.allclose(img1.cpu().numpy(), img0.cpu().numpy(), rtol=1e-9, atol=0)
+
+
+def test_counters_wait_for_the_context_only_and_shard_is_committed_after_its_table(rb):
+    s = scenes.config_C0(32)
+    with rb.Raptor(s) as R:
+        R.render(want_status=False)
+        steps, sampled, rays = R.counters()                                    # no torch synchronize before: the call waits
+        assert rays == 32 * 32 and steps > 100 * rays and 0 < sampled <= steps
+        with pytest.raises(rb.RaptorError):
+            R.set_shard(3, 2)                                                  # refused: previous shard (0, 1) stays
+        full = R.render(want_status=False).cpu().numpy()
+        R.set_shard(1, 2)
+        part = R.render(want_status=False, image=torch.zeros((1, 32, 32), dtype=torch.float64, device="cuda")).cpu().numpy()
+        R.set_shard(0, 1)
+        torch.cuda.synchronize()
+        owned = part != 0.0
+        assert 0 < owned.sum() < owned.size and np.array_equal(part[owned], full[owned])
+        assert R.counters()[2] == 32 * 32 * 2 + 16 * 32          # rank 1 of 2 owns 16 of the 32 8x4-pixel tiles
+
+
+def test_grid_cells_with_denormal_huge_or_infinite_values_hold_no_plasma(rb):
+    # user-supplied grid data reaches the one-step reciprocals of the sampler, which want positive normal arguments;
+    # cells outside (1e-300, 1e300) in density, or with an infinite velocity, are treated as empty instead of
+    # poisoning the ray with NaN (compute-sanitizer is closed on this pool, the oracle divides in IEEE: no parity here)
+    clean = scenes.config_C2(nx=48, n1=32, n2=32)
+    g = np.array(clean.grid, dtype=np.float64, copy=True).reshape(32, 32, 8)
+    g[6:12, 10:16, 0] = 4e-310            # denormal density
+    g[14:20, 12:18, 0] = 1e305            # density beyond the range
+    g[20:25, 14:20, 2] = np.inf           # infinite radial velocity
+    g[8:12, 20:24, 0] = 0.0               # empty cells were always allowed
+    with rb.Raptor(clean) as R:
+        ref, st0, _ = R.render()
+        ref = ref.cpu().numpy()
+        R.upload_grid(g.reshape(clean.grid.shape))
+        img, st1, _ = R.render()
+        img, st1 = img.cpu().numpy(), st1.cpu().numpy()
+    assert np.all(np.isfinite(img)) and np.all(img >= 0.0)
+    assert not np.any(st1 == 5)                                   # RAPTOR_NONFINITE
+    changed = img != ref
+    assert 0 < changed.sum() < changed.size                        # the patched cells matter to some rays, not to all
+    s32 = scenes.config_PB1_f32(nx=48, n1=32, n2=32)
+    with rb.Raptor(s32) as R:
+        R.upload_grid(g.reshape(s32.grid.shape))
+        img32 = R.render(want_status=False).cpu().numpy()
+    assert np.all(np.isfinite(img32))

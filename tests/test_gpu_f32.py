@@ -103,7 +103,7 @@ def test_f32_is_refused_outside_the_papers_configuration(rb):
     s = scenes.config_PB1_f32(nx=8)
     with rb.Raptor(s) as R:
         buf = torch.zeros((64,), dtype=torch.float64, device="cuda")
-        rb.raptor_set_null_monitor(R.ctx, buf.data_ptr())
+        rb.raptor_set_null_monitor(R.ctx, buf.data_ptr(), buf.numel())
         with pytest.raises(rb.RaptorError):
             R.render()
         rb.raptor_set_null_monitor(R.ctx, None)

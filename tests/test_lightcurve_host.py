@@ -76,6 +76,21 @@ def test_calibrate_delay_recovers_a_known_shift():
     assert lc.calibrate_delay(tf, Ff, ts + 100.0, Fs, 0.5, 11) == (0.0, math.inf)
 
 
+def test_calibrate_delay_refuses_curves_it_cannot_normalise_or_interpolate():
+    # a zero mean would normalise to inf/nan and a time axis that is not ascending has no interpolation interval:
+    # both used to come back as (0, inf) "no shift qualified"; now they are errors with a message
+    from paper_1801_10452_b200 import binding
+    t = np.linspace(0.0, 10.0, 21)
+    F = 1.0 + 0.1 * np.sin(t)
+    zero_mean = np.array([1.0, -1.0] * 10 + [0.0])
+    for args in ((t, zero_mean, t, F), (t, F, t, np.zeros_like(F)), (t, F, t[::-1].copy(), F),
+                 (t, F, np.concatenate([t[:5], t[4:-1]]), F)):
+        with pytest.raises(binding.RaptorError) as err:
+            binding.raptor_calibrate_delay(*args, 1.0, 11)
+        assert err.value.code == binding.EINVAL and "raptor_calibrate_delay" in str(err.value)
+    assert binding.raptor_calibrate_delay(t, F, t, 2.0 * F, 1.0, 11)[0] == 0.0
+
+
 def _free_port():
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
