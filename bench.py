@@ -16,6 +16,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import statistics
 import subprocess
@@ -320,6 +321,14 @@ def run_ours(args):
             "config": {"workload": args.workload, "pixels": [scene.nx, scene.ny], "n_freq": scene.n_freq,
                        "spin": scene.a, "incl_deg": scene.incl_deg, "plasma_model": scene.plasma_model,
                        "grid": [scene.nt, scene.n1, scene.n2, scene.n3], "l2": "flushed between timed iterations",
+                       "integrator": ["RK4", "Verlet", "Verlet+corrector", "RK2 (midpoint)"][scene.integrator],
+                       "step_policy": "A" if scene.step_policy == 0 else "B",
+                       "step_rule": (f"h = min(clamp({scene.step_c} (r - r_H), {scene.step_min}, {scene.step_max}), "
+                                     f"eps_polar r |sin theta|), eps_polar = {scene.eps_polar} (polar guard: DESIGN.md 3.2; "
+                                     "BASELINE.json configs[0] states the clamp alone)") if scene.step_policy == 0
+                                    else f"Eq. 21-24, eps = {scene.eps}, delta = {scene.delta}",
+                       "eps_polar": scene.eps_polar if scene.step_policy == 0 else None,
+                       "tau_cutoff": scene.tau_cutoff if math.isfinite(scene.tau_cutoff) else None,
                        "parallelism": ("single GPU" if world == 1 else
                                        f"one image, interleaved 8x4 tiles over {world} ranks + all-reduce(SUM) of the image" if strong
                                        else f"frames x{world}: every rank renders its own frame, no data-path collective")},
@@ -347,10 +356,13 @@ def run_ours(args):
             flop_step = 2.0 * row["ffma"] + row["fmul"] + row["fadd"]
             steps_launch = steps_done / args.steps
             achieved = steps_launch * flop_step / (avg_render_ms * 1e-3) / 1e12
-            peak32 = 148 * 128 * 2 * 1.965e9 / 1e12
+            peak32_nominal = 148 * 128 * 2 * 1.965e9 / 1e12
+            peak32 = binding.raptor_fp32_peak(1 << 16)[0]               # measured here, after the timed region
             line["roofline"] = {
                 "bound": "alu", "kernel": "k_render_f32", "achieved": achieved, "peak": peak32, "unit": "TFLOP/s",
-                "frac": achieved / peak32, "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (no measured FP32 peak)",
+                "frac": achieved / peak32,
+                "peak_source": "measured: raptor_fp32_peak (independent FFMA chains on all SMs) in this process",
+                "peak_nominal": peak32_nominal, "frac_of_nominal": achieved / peak32_nominal,
                 "traffic": (row.get("dram_read_bytes", 0.0) + row.get("dram_write_bytes", 0.0)) if "dram_read_bytes" in row else None,
                 "fp32_inst_per_step": {"ffma": row["ffma"], "fmul": row["fmul"], "fadd": row["fadd"]},
                 "counts_source": "profiles/fp64_inst_per_step.json (ncu, source hash verified)",

@@ -252,6 +252,10 @@ int raptor_get_counters(raptor_ctx *ctx, uint64_t *total_steps, uint64_t *sample
  * *tflops = 2 * FMAs / time.  iters = chain length per thread (e.g. 1<<16). Synchronous. */
 int raptor_fp64_peak(int32_t iters, double *tflops, double *ms);
 
+/* The same for the FP32 FMA pipe (16 independent FFMA chains per thread): the denominator of the roofline of the
+ * single-precision kernel (precision = 1).  Synchronous. */
+int raptor_fp32_peak(int32_t iters, double *tflops, double *ms);
+
 /* Issue rate of the FP64 pipe by operand form (independent chains on all SMs, 8 warps per sub-partition):
  * form 0 fma(x, imm, imm); 1 fma(y, z, x) = three different register sources; 2 fma(x, y, x); 3 x * y; 4 x + z.
  * *warp_inst_per_sec = warp-level instructions per second over the whole device; *sm_clock_hz (may be NULL) = the

@@ -24,7 +24,7 @@ STATUS = {0: "RUNNING", 1: "CAPTURED", 2: "ESCAPED", 3: "MAXSTEPS", 4: "THICK", 
 SYMBOLS = ("raptor_create", "raptor_upload_grid", "raptor_set_shard", "raptor_render", "raptor_render_disk",
            "raptor_line_profile", "raptor_set_camera_time", "raptor_set_window", "raptor_upload_snapshot",
            "raptor_light_curve", "raptor_calibrate_delay", "raptor_spectrum", "raptor_flux", "raptor_flux_static",
-           "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_null_norm", "raptor_set_null_monitor", "raptor_get_counters", "raptor_fp64_peak", "raptor_fp64_probe",
+           "raptor_render_host", "raptor_trace", "raptor_eval_rhs", "raptor_null_norm", "raptor_set_null_monitor", "raptor_get_counters", "raptor_fp64_peak", "raptor_fp32_peak", "raptor_fp64_probe",
            "raptor_destroy", "raptor_last_error")
 
 
@@ -88,6 +88,7 @@ def lib():
         L.raptor_set_null_monitor.argtypes = [vp, vp, C.c_uint64]
         L.raptor_get_counters.argtypes = [vp, u64p, u64p, u64p]
         L.raptor_fp64_peak.argtypes = [i32, dp, dp]
+        L.raptor_fp32_peak.argtypes = [i32, dp, dp]
         L.raptor_fp64_probe.argtypes = [i32, i32, dp, dp]
         L.raptor_destroy.argtypes = [vp]
         L.raptor_last_error.argtypes = [vp]
@@ -233,6 +234,13 @@ def raptor_get_counters(ctx):
 def raptor_fp64_peak(iters: int = 1 << 16):
     tf, ms = C.c_double(), C.c_double()
     _check(lib().raptor_fp64_peak(int(iters), C.byref(tf), C.byref(ms)))
+    return tf.value, ms.value
+
+
+def raptor_fp32_peak(iters: int = 1 << 16):
+    """(TFLOP/s, ms) of independent FFMA chains on all SMs: the measured FP32 peak (raptor.h)."""
+    tf, ms = C.c_double(), C.c_double()
+    _check(lib().raptor_fp32_peak(int(iters), C.byref(tf), C.byref(ms)))
     return tf.value, ms.value
 
 

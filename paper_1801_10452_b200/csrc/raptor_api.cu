@@ -704,6 +704,36 @@ extern "C" int raptor_fp64_peak(int32_t iters, double* tflops, double* ms) {
     return RAPTOR_OK;
 }
 
+extern "C" int raptor_fp32_peak(int32_t iters, double* tflops, double* ms) {
+    if (iters < 1 || !tflops) return fail(nullptr, RAPTOR_EINVAL, "iters < 1 or tflops NULL");
+    int dev = 0, sms = 0;
+    CK(nullptr, cudaGetDevice(&dev));
+    CK(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float* d_out = nullptr;
+    CK(nullptr, cudaMalloc(&d_out, sizeof(float)));
+    cudaEvent_t e0, e1;
+    CK(nullptr, cudaEventCreate(&e0));
+    CK(nullptr, cudaEventCreate(&e1));
+    const int blocks = sms * 8;
+    float best = 1e30f;
+    cudaError_t err = cudaSuccess;
+    for (int rep = 0; rep < 4 && err == cudaSuccess; ++rep) {       // rep 0 warms up
+        cudaEventRecord(e0, 0);
+        err = launch_fp32_peak(iters, blocks, d_out, 0);
+        cudaEventRecord(e1, 0);
+        if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+        float t = 0.f;
+        cudaEventElapsedTime(&t, e0, e1);
+        if (rep > 0 && t < best) best = t;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+    if (err != cudaSuccess) return fail(nullptr, RAPTOR_ECUDA, "fp32 probe: %s", cudaGetErrorString(err));
+    const double flops = 2.0 * 16.0 * (double)iters * 256.0 * (double)blocks;
+    *tflops = flops / (best * 1e-3) * 1e-12;
+    if (ms) *ms = best;
+    return RAPTOR_OK;
+}
+
 extern "C" int raptor_fp64_probe(int32_t form, int32_t iters, double* warp_inst_per_sec, double* sm_clock_hz) {
     if (form < 0 || form > 4 || iters < 1 || !warp_inst_per_sec) return fail(nullptr, RAPTOR_EINVAL, "form 0..4, iters >= 1, output not NULL");
     int dev = 0, sms = 0, khz = 0;

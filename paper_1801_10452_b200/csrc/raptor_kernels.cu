@@ -251,6 +251,28 @@ cudaError_t launch_fp64_form(int mode, int iters, int blocks, double* d_out, cud
     return cudaGetLastError();
 }
 
+// FP32 peak probe (denominator of the single-precision kernel's roofline): 16 independent FFMA chains per thread
+__global__ void __launch_bounds__(256) k_fp32_peak(int iters, float seed, float* __restrict__ out) {
+    float x[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = seed + (float)threadIdx.x + (float)i;
+    const float m = 0.999999f, c = 1e-6f;
+#pragma unroll 2
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = fmaf(x[i], m, c);
+    }
+    float s = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += x[i];
+    if (s == 123.456f) out[0] = s;     // never true; keeps the chains alive
+}
+
+cudaError_t launch_fp32_peak(int iters, int blocks, float* d_out, cudaStream_t stream) {
+    k_fp32_peak<<<blocks, 256, 0, stream>>>(iters, 1.0f, d_out);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_fp64_peak(int iters, int blocks, double* d_out, cudaStream_t stream) {
     k_fp64_peak<<<blocks, 256, 0, stream>>>(iters, 1.0, d_out);
     return cudaGetLastError();

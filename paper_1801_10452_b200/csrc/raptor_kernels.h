@@ -69,6 +69,7 @@ constexpr int kFluxStaticSlots = 16384;      // partial sums the array holds: n_
 cudaError_t launch_flux_static(const double* d_image, size_t npix, int n_planes, double scale, double* d_flux,
                                cudaStream_t stream);
 cudaError_t launch_fp64_peak(int iters, int blocks, double* d_out, cudaStream_t stream);
+cudaError_t launch_fp32_peak(int iters, int blocks, float* d_out, cudaStream_t stream);
 cudaError_t launch_fp64_form(int mode, int iters, int blocks, double* d_out, cudaStream_t stream);
 
 }  // namespace raptor

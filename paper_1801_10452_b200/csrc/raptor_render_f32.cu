@@ -151,7 +151,9 @@ __device__ __forceinline__ bool transfer(const KPf& P, const Geomf& G, const flo
     const float Ur = G.ex * q[2], Uh = G.dth * q[3], Up = q[4];
     const float Br = G.ex * q[5], Bh = G.dth * q[6], Bp = q[7];
     const float opf = 1.0f + M.f, ialpha = sqrtf(opf);
-    const float gam = sqrtf(1.0f + ks_dot(M, 0.0f, Ur, Uh, Up, 0.0f, Ur, Uh, Up));
+    const float qq = ks_dot(M, 0.0f, Ur, Uh, Up, 0.0f, Ur, Uh, Up);
+    if (!(qq < 1e30f)) return false;                                            // infinite or NaN velocity in the cell: no plasma
+    const float gam = sqrtf(1.0f + qq);
     const float ut = gam * ialpha, ur = fmaf(-gam * ialpha, M.f * rcpf(opf), Ur), uh = Uh, up = Up;
     const float bt = ks_dot(M, 0.0f, Br, Bh, Bp, ut, ur, uh, up);
     const float iut = rcpf(ut);

@@ -11,11 +11,14 @@ The oracle needs about twelve minutes of host time on 16 cores for these images 
 RAPTOR_FULL_PARITY_ROWS=k restricts every image to each k-th row (development runs only; the report says so).
 The oracle's time is budgeted (RAPTOR_FULL_PARITY_BUDGET_S, default 840 s) so that a slower host degrades to every 2nd,
 3rd ... row of the images still to come instead of running into the time limit of the whole GPU test run; the report
-names the stride of every image, and the committed report is from a run with stride 1 throughout.
+names the stride of every image, a thinned image raises a warning, and the last test puts a one-line summary (strides,
+pixel count, worst errors) into pytest's warnings summary, so the tail of a -q run says what was compared; the committed
+report is from a run with stride 1 throughout.
 The report is written to gpurun_out/parity_full.md; the committed copy is profiles/parity_full_r2.md.
 """
 import os
 import time
+import warnings
 
 import numpy as np
 import pytest
@@ -111,6 +114,10 @@ def test_whole_image_parity_at_full_size(name):
     t_oracle = time.perf_counter() - t0
     CLOCK["elapsed"] += t_oracle
     CLOCK["steps"] += float(ref["steps"])
+    if stride != ROW_STRIDE:
+        # never silently: a thinned comparison shows up in pytest's warnings summary (also under -q)
+        warnings.warn(f"full parity: {name} compared on every {stride}th row only (oracle time budget {BUDGET_S:.0f} s, "
+                      f"{CLOCK['elapsed']:.0f} s used)")
     rows = np.arange(stride // 2, scene.ny, stride)
     ref_flux = o.flux(ref["image"]) if stride == 1 else None
     rep = _report_row(name, scene, g, ref, ref_flux, rows, t_oracle, stride)
@@ -172,3 +179,10 @@ def test_zz_slow_vs_fast_light_and_write_report():
     except OSError:
         pass
     print("\n".join(lines))
+    # one line for the tail of the run (pytest -q prints warnings, not captured output): what was compared, and how well
+    rows_ = [r for r in REPORT.values() if isinstance(r, dict)]
+    full = sum(1 for r in rows_ if r["row_stride"] == 1)
+    warnings.warn(f"full parity summary: stride 1 on {full}/{len(rows_)} images (strides "
+                  f"{[r['row_stride'] for r in rows_]}), {sum(r['pixels'] * len(r['flux_err_all']) for r in rows_)} pixel values outside the band, "
+                  f"min frac(err <= 1e-8) = {min(r['frac_ok'] for r in rows_):.6f}, max err = {max(r['max_err'] for r in rows_):.2e}, "
+                  f"max flux err = {max(r['flux_err_max'] for r in rows_):.2e}, oracle {CLOCK['elapsed']:.0f} s")

@@ -237,6 +237,23 @@ def test_policy_A_without_the_polar_guard_is_the_literal_baseline_rule(rb, orc):
     assert abs(fg - fo) <= 1e-9 * abs(fo)
 
 
+def test_literal_baseline_rule_on_the_grid_configuration(rb, orc):
+    # the same literal rule (no polar guard) on BASELINE.json configs[2] at small size: Kerr, MKS h = 0.3, 20 deg
+    # inclination, so many rays pass close to the axis; rays that end NONFINITE do so on both sides alike
+    s = replace(scenes.config_C2(nx=48, n1=64, n2=64), eps_polar=1e30)
+    g = gpu_render(rb, s)
+    ref = orc.Oracle(s).render()
+    bad = (ref["status"] == 5) | (g["status"] == 5)
+    keep = ~ring_mask(s) & ~bad
+    assert bad.sum() <= 0.05 * bad.size
+    assert np.array_equal(g["status"][keep], ref["status"][keep])
+    assert (g["nsteps"][keep] == ref["nsteps"][keep]).mean() >= 0.999
+    err = rel_err(g["image"], ref["image"])[0]
+    assert (err[keep] <= 1e-8).mean() >= 0.999
+    fo, fg = ref["image"][0][keep].sum(), g["image"][0][keep].sum()
+    assert abs(fg - fo) <= 1e-8 * abs(fo)
+
+
 def test_multi_frequency_path_equals_single_frequency_path(rb):
     s3 = scenes.config_C3(nx=16, n_freq=4)
     g3 = gpu_render(rb, s3)
