@@ -14,7 +14,7 @@ The oracle's time is budgeted (RAPTOR_FULL_PARITY_BUDGET_S, default 840 s) so th
 names the stride of every image, a thinned image raises a warning, and the last test puts a one-line summary (strides,
 pixel count, worst errors) into pytest's warnings summary, so the tail of a -q run says what was compared; the committed
 report is from a run with stride 1 throughout.
-The report is written to gpurun_out/parity_full.md; the committed copy is profiles/parity_full_r2.md.
+The report is written to gpurun_out/parity_full.md; the committed copy is profiles/parity_full_r3.md.
 """
 import os
 import time
